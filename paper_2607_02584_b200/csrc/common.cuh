@@ -1,0 +1,62 @@
+// Shared host/device declarations of librotattn (not part of the public ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "rotattn.h"
+
+namespace rotattn {
+
+constexpr int kTile = 128;        // query tile = KV block = V group (readings 11, 18)
+constexpr int kQKRowBytes = 128;  // widened int8 Q/K rows are always 128 B (D=64 rows are zero-padded)
+
+inline __host__ __device__ int ceil_div(int a, int b) { return (a + b - 1) / b; }
+inline __host__ __device__ size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// Layout of the INT4-path workspace (rotattn_workspace_bytes(p, 0)).
+struct WsInt4 {
+  size_t q8, k8, v8t, total;
+  int npad;
+  __host__ explicit WsInt4(const rotattn_params& p) {
+    size_t bh = (size_t)p.B * p.H;
+    npad = ceil_div(p.N, kTile) * kTile;
+    size_t qk = align_up(bh * (size_t)p.N * kQKRowBytes, 1024);
+    q8 = 0;
+    k8 = q8 + qk;
+    v8t = k8 + qk;
+    total = v8t + align_up(bh * (size_t)p.D * npad, 1024);
+  }
+};
+
+// FP16-path workspace: V transposed [BH, D, npad] fp16.
+struct WsFp16 {
+  size_t vt, total;
+  int npad;
+  __host__ explicit WsFp16(const rotattn_params& p) {
+    size_t bh = (size_t)p.B * p.H;
+    npad = ceil_div(p.N, kTile) * kTile;
+    vt = 0;
+    total = align_up(bh * (size_t)p.D * npad * 2, 1024);
+  }
+};
+
+// error plumbing
+void set_cuda_error(cudaError_t e, const char* where);
+void set_error_text(const char* text);
+int check_device_sm100();   // ROTATTN_OK or ROTATTN_ERR_UNSUPPORTED / ROTATTN_ERR_CUDA
+
+#define ROTATTN_CUDA_TRY(expr)                                   \
+  do {                                                           \
+    cudaError_t _e = (expr);                                     \
+    if (_e != cudaSuccess) {                                     \
+      ::rotattn::set_cuda_error(_e, #expr);                      \
+      return ROTATTN_ERR_CUDA;                                   \
+    }                                                            \
+  } while (0)
+
+// internal launchers (prologue.cu)
+int launch_unpack_qk(const rotattn_params& p, const uint8_t* X4, int8_t* X8, cudaStream_t st);
+int launch_unpack_vt(const rotattn_params& p, const uint8_t* V4, int8_t* V8T, int npad, cudaStream_t st);
+
+}  // namespace rotattn

@@ -1,0 +1,368 @@
+// Prologue kernels (HBM-bound): prepare_qk (a1+a2), quant_v (a3) and the unpack helpers.
+// Code-producing arithmetic is fp32 with one rounding per operation (__fmul_rn/__fadd_rn/__fdiv_rn,
+// never contracted) so that the INT4 codes are reproducible bit for bit ("bit-exact prologue").
+#include "common.cuh"
+
+namespace rotattn {
+
+// ------------------------------------------------------------------------------------------------
+// prepare_qk: one warp per token; lane l owns channels [CPL*l, CPL*l+CPL) of Q and of K.
+// ------------------------------------------------------------------------------------------------
+struct PrepArgs {
+  const __half* X[2];     // Q, K  [BH*N, D]
+  uint8_t* X4[2];         // packed codes [BH*N, D/2]
+  float* Xs[2];           // scales [BH*N]
+  __half* X16[2];         // optional fp16 y
+  int8_t* X8[2];          // optional widened codes [BH*N, 128]
+  const float4* coef;     // table rows
+  const float4* rot;      // [D/2] blocks or nullptr (H_2)
+  long long total;        // BH*N tokens
+  int N, n_rope, gt, gh, gw, Pt, Ph, Pw;
+};
+
+__device__ __forceinline__ int quant_code(float y, float inv) {
+  int c = __float2int_rn(__fmul_rn(y, inv));       // round half to even
+  return max(-7, min(7, c));
+}
+
+template <int D, int ROT>
+__global__ void __launch_bounds__(256) prepare_qk_kernel(const PrepArgs a) {
+  constexpr int CPL = D / 32;       // channels per lane
+  constexpr int PPL = CPL / 2;      // RoPE pairs per lane
+  constexpr int WPB = 8;            // warps per block
+  __shared__ float ybuf[WPB][2][D]; // HALF-rotation exchange buffer
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+
+  // ---- per-lane constants ----
+  int cbase[PPL], cstride[PPL], caxis[PPL];
+  {
+    const int secbase[3] = {0, (a.gt + 1) * a.Pt, (a.gt + 1) * a.Pt + (a.gh + 1) * a.Ph};
+#pragma unroll
+    for (int i = 0; i < PPL; ++i) {
+      int g = lane * PPL + i;
+      int ax = g < a.Pt ? 0 : (g < a.Pt + a.Ph ? 1 : 2);
+      int k = g - (ax == 0 ? 0 : (ax == 1 ? a.Pt : a.Pt + a.Ph));
+      int P = ax == 0 ? a.Pt : (ax == 1 ? a.Ph : a.Pw);
+      caxis[i] = ax; cbase[i] = secbase[ax] + k; cstride[i] = P;
+    }
+  }
+  int partner[CPL]; float ca[CPL], cb[CPL]; bool role_u[CPL];
+  if (ROT == ROTATTN_ROT_HALF) {
+#pragma unroll
+    for (int j = 0; j < CPL; ++j) {
+      int c = lane * CPL + j;
+      int sec = c < 2 * a.Pt ? 0 : (c < 2 * (a.Pt + a.Ph) ? 1 : 2);
+      int o = sec == 0 ? 0 : (sec == 1 ? 2 * a.Pt : 2 * (a.Pt + a.Ph));
+      int P = sec == 0 ? a.Pt : (sec == 1 ? a.Ph : a.Pw);
+      int goff = o / 2;
+      int i = c - o;
+      role_u[j] = i < P;
+      int blk = goff + (role_u[j] ? i : i - P);
+      partner[j] = role_u[j] ? c + P : c - P;
+      float4 r = a.rot ? a.rot[blk] : make_float4(0.70710678118654752440f, 0.70710678118654752440f,
+                                                  0.70710678118654752440f, -0.70710678118654752440f);
+      ca[j] = role_u[j] ? r.x : r.y;   // multiplies u
+      cb[j] = role_u[j] ? r.z : r.w;   // multiplies v
+    }
+  }
+
+  const long long wstride = (long long)gridDim.x * WPB;
+  for (long long tok = (long long)blockIdx.x * WPB + warp; tok < a.total; tok += wstride) {
+    const int n = (int)(tok % a.N);
+    int pos[3];
+    if (n < a.n_rope) {
+      pos[2] = n % a.gw; int r = n / a.gw; pos[1] = r % a.gh; pos[0] = r / a.gh;
+    } else {
+      pos[0] = a.gt; pos[1] = a.gh; pos[2] = a.gw;     // no-RoPE rows
+    }
+    float4 A[PPL];
+#pragma unroll
+    for (int i = 0; i < PPL; ++i) A[i] = __ldg(a.coef + cbase[i] + pos[caxis[i]] * cstride[i]);
+
+    float y[2][CPL];
+#pragma unroll
+    for (int m = 0; m < 2; ++m) {
+      const __half* src = a.X[m] + tok * D + lane * CPL;
+      __half hx[CPL];
+      if (CPL == 4) { uint2 v = *reinterpret_cast<const uint2*>(src); *reinterpret_cast<uint2*>(hx) = v; }
+      else { uint32_t v = *reinterpret_cast<const uint32_t*>(src); *reinterpret_cast<uint32_t*>(hx) = v; }
+#pragma unroll
+      for (int i = 0; i < PPL; ++i) {
+        float x0 = __half2float(hx[2 * i]), x1 = __half2float(hx[2 * i + 1]);
+        y[m][2 * i]     = __fadd_rn(__fmul_rn(x0, A[i].x), __fmul_rn(x1, A[i].z));
+        y[m][2 * i + 1] = __fadd_rn(__fmul_rn(x0, A[i].y), __fmul_rn(x1, A[i].w));
+      }
+    }
+    if (ROT == ROTATTN_ROT_HALF) {
+#pragma unroll
+      for (int m = 0; m < 2; ++m)
+#pragma unroll
+        for (int j = 0; j < CPL; ++j) ybuf[warp][m][lane * CPL + j] = y[m][j];
+      __syncwarp();
+#pragma unroll
+      for (int m = 0; m < 2; ++m)
+#pragma unroll
+        for (int j = 0; j < CPL; ++j) {
+          float other = ybuf[warp][m][partner[j]];
+          float u = role_u[j] ? y[m][j] : other;
+          float v = role_u[j] ? other : y[m][j];
+          y[m][j] = __fadd_rn(__fmul_rn(u, ca[j]), __fmul_rn(v, cb[j]));
+        }
+      __syncwarp();
+    }
+#pragma unroll
+    for (int m = 0; m < 2; ++m) {
+      float amax = 0.f;
+#pragma unroll
+      for (int j = 0; j < CPL; ++j) amax = fmaxf(amax, fabsf(y[m][j]));
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+      const float scale = __fdiv_rn(amax, 7.0f);
+      const float inv = amax > 0.f ? __fdiv_rn(7.0f, amax) : 0.f;
+      int c[CPL];
+#pragma unroll
+      for (int j = 0; j < CPL; ++j) c[j] = quant_code(y[m][j], inv);
+      if (CPL == 4) {
+        uint16_t pk = (uint16_t)((c[0] & 0xF) | ((c[1] & 0xF) << 4) | ((c[2] & 0xF) << 8) | ((c[3] & 0xF) << 12));
+        *reinterpret_cast<uint16_t*>(a.X4[m] + tok * (D / 2) + lane * 2) = pk;
+      } else {
+        a.X4[m][tok * (D / 2) + lane] = (uint8_t)((c[0] & 0xF) | ((c[1] & 0xF) << 4));
+      }
+      if (lane == 0) a.Xs[m][tok] = scale;
+      if (a.X8[m]) {
+        int8_t* dst = a.X8[m] + tok * kQKRowBytes;
+        if (CPL == 4) {
+          uint32_t w = (uint32_t)(c[0] & 0xFF) | ((uint32_t)(c[1] & 0xFF) << 8) | ((uint32_t)(c[2] & 0xFF) << 16) | ((uint32_t)(c[3] & 0xFF) << 24);
+          *reinterpret_cast<uint32_t*>(dst + lane * 4) = w;
+        } else {
+          *reinterpret_cast<uint16_t*>(dst + lane * 2) = (uint16_t)((c[0] & 0xFF) | ((c[1] & 0xFF) << 8));
+          *reinterpret_cast<uint16_t*>(dst + 64 + lane * 2) = 0;      // zero pad to a 128-byte row
+        }
+      }
+      if (a.X16[m]) {
+        __half* dst = a.X16[m] + tok * D + lane * CPL;
+        __half hy[CPL];
+#pragma unroll
+        for (int j = 0; j < CPL; ++j) hy[j] = __float2half_rn(y[m][j]);
+        if (CPL == 4) *reinterpret_cast<uint2*>(dst) = *reinterpret_cast<uint2*>(hy);
+        else *reinterpret_cast<uint32_t*>(dst) = *reinterpret_cast<uint32_t*>(hy);
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// quant_v: one CTA per (bh, group of 128 tokens).  V is read once into registers; the per-channel
+// amax is reduced through shuffles + shared memory; codes go out packed [N, D/2] and, transposed
+// through a swizzled shared tile, as int8 [D, npad] (K-major B operand of the P~V MMA).
+// ------------------------------------------------------------------------------------------------
+template <int D>
+__global__ void __launch_bounds__(256) quant_v_kernel(const __half* __restrict__ V, uint8_t* __restrict__ V4,
+                                                      float* __restrict__ Vs, int8_t* __restrict__ V8T,
+                                                      int N, int nG, int npad) {
+  constexpr int CR = D / 8;           // 16-byte chunks per row
+  constexpr int QPP = 256 / CR;       // row-quads per pass
+  constexpr int NPASS = 32 / QPP;     // passes over the 32 row-quads
+  constexpr int SW = 32 / CR;         // swizzle multiplier
+  __shared__ float amax_s[8][CR][8];
+  __shared__ uint32_t tileT[D][32];
+  const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+  const int cc = t % CR, q0 = t / CR;
+  const int g = blockIdx.x % nG;
+  const long long bh = blockIdx.x / nG;
+  const int row0 = g * kTile;
+  const __half* base = V + (bh * N + row0) * (long long)D + cc * 8;
+
+  uint4 raw[NPASS][4];
+#pragma unroll
+  for (int ps = 0; ps < NPASS; ++ps)
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      int row = (q0 + ps * QPP) * 4 + r;
+      raw[ps][r] = (row0 + row < N) ? __ldg(reinterpret_cast<const uint4*>(base + (long long)row * D)) : make_uint4(0, 0, 0, 0);
+    }
+  float am[8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) am[j] = 0.f;
+#pragma unroll
+  for (int ps = 0; ps < NPASS; ++ps)
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      const __half* h = reinterpret_cast<const __half*>(&raw[ps][r]);
+#pragma unroll
+      for (int j = 0; j < 8; ++j) am[j] = fmaxf(am[j], fabsf(__half2float(h[j])));
+    }
+#pragma unroll
+  for (int o = CR; o < 32; o <<= 1)
+#pragma unroll
+    for (int j = 0; j < 8; ++j) am[j] = fmaxf(am[j], __shfl_xor_sync(0xffffffffu, am[j], o));
+  if (lane < CR) {
+#pragma unroll
+    for (int j = 0; j < 8; ++j) amax_s[warp][cc][j] = am[j];
+  }
+  __syncthreads();
+  float inv[8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    float m = 0.f;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) m = fmaxf(m, amax_s[w][cc][j]);
+    inv[j] = m > 0.f ? __fdiv_rn(7.0f, m) : 0.f;
+    if (t < CR) Vs[(bh * nG + g) * D + cc * 8 + j] = __fdiv_rn(m, 7.0f);
+  }
+#pragma unroll
+  for (int ps = 0; ps < NPASS; ++ps) {
+    uint32_t tw[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) tw[j] = 0;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      const __half* h = reinterpret_cast<const __half*>(&raw[ps][r]);
+      uint32_t pk = 0;
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        int c = quant_code(__half2float(h[j]), inv[j]);
+        pk |= (uint32_t)(c & 0xF) << (4 * j);
+        tw[j] |= (uint32_t)(c & 0xFF) << (8 * r);
+      }
+      int row = (q0 + ps * QPP) * 4 + r;
+      if (row0 + row < N) *reinterpret_cast<uint32_t*>(V4 + (bh * N + row0 + row) * (long long)(D / 2) + cc * 4) = pk;
+    }
+    if (V8T) {
+      const int word = q0 + ps * QPP;
+#pragma unroll
+      for (int j = 0; j < 8; ++j) tileT[cc * 8 + j][(word ^ (SW * cc)) & 31] = tw[j];
+    }
+  }
+  if (V8T) {
+    __syncthreads();
+    for (int ch = warp; ch < D; ch += 8) {
+      uint32_t w = tileT[ch][(lane ^ (SW * (ch / 8))) & 31];
+      *reinterpret_cast<uint32_t*>(V8T + (bh * D + ch) * (long long)npad + row0 + lane * 4) = w;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// unpack helpers: rebuild the widened copies from the packed public buffers (fresh workspace).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ int nib2int(uint32_t nib) { return (int)((nib ^ 8u) & 0xFu) - 8; }
+
+__global__ void unpack_qk_kernel(const uint8_t* __restrict__ X4, int8_t* __restrict__ X8, long long tokens, int D) {
+  // one thread per output 4-byte word
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long total = tokens * (kQKRowBytes / 4);
+  if (idx >= total) return;
+  const long long tok = idx / (kQKRowBytes / 4);
+  const int w = (int)(idx % (kQKRowBytes / 4));
+  uint32_t out = 0;
+  if (w * 4 < D) {
+    const uint16_t pk = *reinterpret_cast<const uint16_t*>(X4 + tok * (D / 2) + w * 2);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) out |= (uint32_t)(nib2int((pk >> (4 * j)) & 0xF) & 0xFF) << (8 * j);
+  }
+  *reinterpret_cast<uint32_t*>(X8 + tok * kQKRowBytes + w * 4) = out;
+}
+
+__global__ void unpack_vt_kernel(const uint8_t* __restrict__ V4, int8_t* __restrict__ V8T, int N, int D, int npad) {
+  // grid: (npad/128, BH); block 256: transposes one 128-token group through shared memory
+  __shared__ int8_t tile[128][128 + 4];
+  const long long bh = blockIdx.y;
+  const int row0 = blockIdx.x * kTile;
+  for (int i = threadIdx.x; i < kTile * (D / 2); i += blockDim.x) {
+    int r = i / (D / 2), b = i % (D / 2);
+    uint8_t pk = (row0 + r < N) ? V4[(bh * N + row0 + r) * (long long)(D / 2) + b] : 0;
+    tile[2 * b][r] = (int8_t)nib2int(pk & 0xF);
+    tile[2 * b + 1][r] = (int8_t)nib2int(pk >> 4);
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < D * kTile; i += blockDim.x) {
+    int ch = i / kTile, r = i % kTile;
+    V8T[(bh * D + ch) * (long long)npad + row0 + r] = tile[ch][r];
+  }
+}
+
+int launch_unpack_qk(const rotattn_params& p, const uint8_t* X4, int8_t* X8, cudaStream_t st) {
+  const long long tokens = (long long)p.B * p.H * p.N;
+  const long long total = tokens * (kQKRowBytes / 4);
+  unpack_qk_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(X4, X8, tokens, p.D);
+  ROTATTN_CUDA_TRY(cudaGetLastError());
+  return ROTATTN_OK;
+}
+
+int launch_unpack_vt(const rotattn_params& p, const uint8_t* V4, int8_t* V8T, int npad, cudaStream_t st) {
+  dim3 grid(npad / kTile, p.B * p.H);
+  unpack_vt_kernel<<<grid, 256, 0, st>>>(V4, V8T, p.N, p.D, npad);
+  ROTATTN_CUDA_TRY(cudaGetLastError());
+  return ROTATTN_OK;
+}
+
+template <int D>
+static int launch_prepare(const rotattn_params& p, const PrepArgs& a, cudaStream_t st) {
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  long long blocks_needed = (a.total + 7) / 8;
+  long long cap = (long long)sms * 8 * 4;          // 8 CTAs of 8 warps per SM, 4 tokens per warp minimum
+  unsigned grid = (unsigned)(blocks_needed < cap ? blocks_needed : cap);
+  if (grid == 0) grid = 1;
+  switch (p.rot_mode) {
+    case ROTATTN_ROT_NONE:
+    case ROTATTN_ROT_INTERLEAVED:   // merged into the table: same kernel as plain RoPE
+      prepare_qk_kernel<D, ROTATTN_ROT_NONE><<<grid, 256, 0, st>>>(a); break;
+    default:
+      prepare_qk_kernel<D, ROTATTN_ROT_HALF><<<grid, 256, 0, st>>>(a); break;
+  }
+  ROTATTN_CUDA_TRY(cudaGetLastError());
+  return ROTATTN_OK;
+}
+
+}  // namespace rotattn
+
+using namespace rotattn;
+
+extern "C" int rotattn_prepare_qk(const rotattn_params* p, const float* coef_dev, const float* rot_dev,
+                                  const void* Q, const void* K, uint8_t* Q4, float* Qs, uint8_t* K4, float* Ks,
+                                  void* Qrope16, void* Krope16, void* workspace, size_t ws_bytes, void* stream) {
+  int st = rotattn_validate(p);
+  if (st != ROTATTN_OK) return st;
+  if (!coef_dev || !Q || !K || !Q4 || !Qs || !K4 || !Ks) return ROTATTN_ERR_INVALID_ARG;
+  if ((st = check_device_sm100()) != ROTATTN_OK) return st;
+  PrepArgs a{};
+  a.X[0] = (const __half*)Q; a.X[1] = (const __half*)K;
+  a.X4[0] = Q4; a.X4[1] = K4; a.Xs[0] = Qs; a.Xs[1] = Ks;
+  a.X16[0] = (__half*)Qrope16; a.X16[1] = (__half*)Krope16;
+  if (workspace) {
+    WsInt4 ws(*p);
+    if (ws_bytes < ws.total) return ROTATTN_ERR_WORKSPACE_TOO_SMALL;
+    a.X8[0] = (int8_t*)workspace + ws.q8; a.X8[1] = (int8_t*)workspace + ws.k8;
+  }
+  a.coef = (const float4*)coef_dev; a.rot = (const float4*)rot_dev;
+  a.total = (long long)p->B * p->H * p->N;
+  a.N = p->N; a.n_rope = p->grid_t * p->grid_h * p->grid_w;
+  a.gt = p->grid_t; a.gh = p->grid_h; a.gw = p->grid_w;
+  a.Pt = p->pairs_t; a.Ph = p->pairs_h; a.Pw = p->pairs_w;
+  return p->D == 128 ? launch_prepare<128>(*p, a, (cudaStream_t)stream) : launch_prepare<64>(*p, a, (cudaStream_t)stream);
+}
+
+extern "C" int rotattn_quant_v(const rotattn_params* p, const void* V, uint8_t* V4, float* Vs,
+                               void* workspace, size_t ws_bytes, void* stream) {
+  int st = rotattn_validate(p);
+  if (st != ROTATTN_OK) return st;
+  if (!V || !V4 || !Vs) return ROTATTN_ERR_INVALID_ARG;
+  if ((st = check_device_sm100()) != ROTATTN_OK) return st;
+  int8_t* v8t = nullptr;
+  WsInt4 ws(*p);
+  if (workspace) {
+    if (ws_bytes < ws.total) return ROTATTN_ERR_WORKSPACE_TOO_SMALL;
+    v8t = (int8_t*)workspace + ws.v8t;
+  }
+  const int nG = ceil_div(p->N, kTile);
+  const unsigned grid = (unsigned)((long long)p->B * p->H * nG);
+  if (p->D == 128)
+    quant_v_kernel<128><<<grid, 256, 0, (cudaStream_t)stream>>>((const __half*)V, V4, Vs, v8t, p->N, nG, ws.npad);
+  else
+    quant_v_kernel<64><<<grid, 256, 0, (cudaStream_t)stream>>>((const __half*)V, V4, Vs, v8t, p->N, nG, ws.npad);
+  ROTATTN_CUDA_TRY(cudaGetLastError());
+  return ROTATTN_OK;
+}

@@ -84,7 +84,7 @@ def outlier_spec(w: Workload, head: int):
         vch = rng.choice(D, size=4, replace=False)
         vsc = np.full(4, 8.0)
     else:
-        counts = (3, 3, 2) if Pt >= 6 else (2, 3, 3)
+        counts = (3, 3, 2) if Pt >= 16 else (2, 3, 3)
         pl = []
         for a, P in enumerate(w.pairs):
             pl += [offs[a] + int(k) for k in rng.choice(_low_freq_half(P), size=counts[a], replace=False)]

@@ -1,0 +1,122 @@
+"""CPU-only tests of the C-ABI host logic: the library loads, exports every declared symbol, validates
+arguments, builds the same coefficient table as the oracle and implements the fallback policy (L192)."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import __graft_entry__ as entry
+
+entry.build()
+from paper_2607_02584_b200 import binding as b  # noqa: E402
+from oracle import rotattn_oracle as orc  # noqa: E402
+from synth import video_qkv as syn  # noqa: E402
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_header_symbols_exported():
+    hdr = open(os.path.join(ROOT, 'include', 'rotattn.h')).read()
+    names = set(re.findall(r'\b(rotattn_[a-z0-9_]+)\s*\(', hdr))
+    assert names == set(b.EXPORTS), names ^ set(b.EXPORTS)
+    for n in names:
+        assert hasattr(b.lib, n)
+
+
+def _p(w, **kw):
+    return b.make_params(w.B, w.H, w.N, w.D, w.grid, w.pairs, **kw)
+
+
+def test_validate_codes():
+    w = syn.TINY
+    assert b.lib.rotattn_validate(C.byref(_p(w))) == 0
+    assert b.lib.rotattn_validate(None) == -1
+    bad = _p(w); bad.pairs_t = 11
+    assert b.lib.rotattn_validate(C.byref(bad)) == -1
+    bad = _p(w); bad.grid_t = 100
+    assert b.lib.rotattn_validate(C.byref(bad)) == -1
+    bad = _p(w); bad.D = 96; bad.pairs_t = 28
+    assert b.lib.rotattn_validate(C.byref(bad)) == -2
+    assert b.lib.rotattn_validate(C.byref(_p(w, kv_block=64))) == -2
+    assert b.lib.rotattn_validate(C.byref(_p(w, qk_group=128))) == -2
+    assert b.lib.rotattn_strerror(-3).decode().startswith('rotation')
+
+
+@pytest.mark.parametrize('w', [syn.TINY, syn.WAN_1_3B, syn.HUNYUAN])
+@pytest.mark.parametrize('mode', [orc.ROT_NONE, orc.ROT_INTERLEAVED, orc.ROT_HALF])
+def test_tables_match_oracle(w, mode):
+    p = _p(w, rot_mode=mode)
+    n = b.lib.rotattn_table_floats(C.byref(p))
+    po = orc.Params(w.B, w.H, w.N, w.D, w.grid, w.pairs, rot_mode=mode)
+    assert n == 4 * orc.table_rows(po)
+    out = np.empty(n, dtype=np.float32)
+    assert b.lib.rotattn_build_tables(C.byref(p), None, out.ctypes.data_as(C.c_void_p)) == 0
+    want = orc.coef_table(po)
+    got = out.reshape(-1, 4)
+    # libm vs NumPy pow/cos may differ in the last fp64 bit; after fp32 rounding that shows only on ties
+    mism = np.count_nonzero(got != want)
+    assert mism <= max(2, got.size // 100000), mism
+    assert np.abs(got - want).max() <= 1.2e-7
+
+
+def test_tables_reject_non_orthogonal_and_accept_random_o2():
+    w = syn.TINY
+    p = _p(w, rot_mode=orc.ROT_INTERLEAVED)
+    out = np.empty(b.lib.rotattn_table_floats(C.byref(p)), dtype=np.float32)
+    rot = orc.default_rot(w.D).astype(np.float32)
+    rot[5] *= 1.01
+    assert b.lib.rotattn_build_tables(C.byref(p), rot.ctypes.data_as(C.c_void_p), out.ctypes.data_as(C.c_void_p)) == -3
+    th = np.random.default_rng(0).uniform(0, 6.28, w.D // 2)
+    rot = np.stack([np.cos(th), np.sin(th), np.sin(th), -np.cos(th)], 1).astype(np.float32)
+    assert b.lib.rotattn_build_tables(C.byref(p), rot.ctypes.data_as(C.c_void_p), out.ctypes.data_as(C.c_void_p)) == 0
+    po = orc.Params(w.B, w.H, w.N, w.D, w.grid, w.pairs, rot_mode=orc.ROT_INTERLEAVED)
+    assert np.abs(out.reshape(-1, 4) - orc.coef_table(po, rot)).max() <= 1.2e-7
+
+
+def test_workspace_sizes():
+    w = syn.WAN_1_3B
+    p = _p(w)
+    npad = -(-w.N // 128) * 128
+    ws0 = b.lib.rotattn_workspace_bytes(C.byref(p), 0)
+    assert ws0 >= 2 * w.H * w.N * 128 + w.H * w.D * npad
+    assert b.lib.rotattn_workspace_bytes(C.byref(p), 1) >= w.H * w.D * npad * 2
+    assert b.lib.rotattn_workspace_bytes(C.byref(p), 7) == 0
+
+
+def test_policy_matches_oracle_and_paper_fractions():
+    for ns, nb, fs, ls, fb, lb in [(40, 40, 6, 4, 2, 2), (40, 40, 2, 2, 2, 2), (50, 60, 4, 2, 2, 2)]:
+        pol = b.RotattnPolicy(ns, nb, fs, ls, fb, lb, None)
+        o = orc.Policy(ns, nb, fs, ls, fb, lb)
+        n = 0
+        for s in range(ns):
+            for k in range(nb):
+                r = b.lib.rotattn_policy_select(C.byref(pol), s, k, 0)
+                assert r == o.select(s, k)
+                n += 1 - r
+        assert n / (ns * nb) == o.int4_fraction()
+    assert b.lib.rotattn_policy_select(C.byref(b.RotattnPolicy(40, 40, 2, 2, 2, 2, None)), 40, 0, 0) == -1
+
+
+def test_policy_split_heads():
+    mask = (C.c_uint8 * 6)(0, 1, 0, 0, 1, 0)
+    pol = b.RotattnPolicy(50, 4, 5, 0, 0, 0, mask)
+    a = np.zeros(12, dtype=np.int32); bb = np.zeros(12, dtype=np.int32)
+    na, nb = C.c_int32(), C.c_int32()
+    args = (a.ctypes.data_as(C.c_void_p), C.cast(C.byref(na), C.c_void_p), bb.ctypes.data_as(C.c_void_p), C.cast(C.byref(nb), C.c_void_p))
+    assert b.lib.rotattn_policy_split_heads(C.byref(pol), 0, 0, 2, 6, *args) == 0
+    assert na.value == 0 and nb.value == 12
+    assert b.lib.rotattn_policy_split_heads(C.byref(pol), 7, 1, 2, 6, *args) == 0
+    assert list(a[:na.value]) == [0, 2, 3, 5, 6, 8, 9, 11] and list(bb[:nb.value]) == [1, 4, 7, 10]
+
+
+def test_compute_entry_points_fail_loudly_without_gpu():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip('GPU present')
+    w = syn.TINY
+    p = _p(w)
+    one = C.c_void_p(16)
+    r = b.lib.rotattn_quant_v(C.byref(p), one, one, one, None, 0, None)
+    assert r in (-2, -5)
