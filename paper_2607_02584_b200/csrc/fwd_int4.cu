@@ -1,11 +1,384 @@
+// rotattn_fwd_int4 (steps a4-a9): INT4 FlashAttention forward on tcgen05 kind::i8.
+//
+// One CTA = one 128-row query tile of one (b,h); 12 warps, warp-specialised:
+//   warp 0      TMA producer   : Q tile once, K / V^T tiles through 3-stage shared-memory rings
+//   warp 1      MMA issuer     : S = Q K^T (int8 x int8 -> int32, TMEM), P~V (u8 from TMEM x int8 -> int32, TMEM)
+//   warp 2      TMEM allocator
+//   warps 4-7   softmax group  : int32 S -> dequant -> block row max -> P^ = exp2 -> codes u = rne(15 P^) -> TMEM
+//   warps 8-11  drain group    : int32 P~V block result -> fp32 O registers (alpha, beta, V scales), epilogue O/l
+// TMEM (512 columns): S[2] at 0/128 (the u8 P tile aliases the first 32 columns of its S buffer), PV[2] at 256/384.
+// The per-block drain is forced by the method: beta (row, block) and Vs (channel, block) change every KV block
+// (PAPER.md:L157 online softmax, L190 per-group V scales), so integer P~V cannot accumulate across blocks.
+#include <cmath>
+#include <cstdio>
 #include "tc_common.cuh"
-using namespace rotattn;
-extern "C" int rotattn_fwd_int4(const rotattn_params* p, const uint8_t*, const float*, const uint8_t*, const float*,
-                                const uint8_t*, const float*, void*, const int32_t*, int32_t, void*, size_t, int32_t, void*) {
-  (void)p; return ROTATTN_ERR_UNSUPPORTED;
+
+namespace rotattn {
+
+constexpr int KV_STAGES = 3;
+constexpr int AB_RING = 4;
+
+struct FwdInt4Args {
+  const float* Qs;        // [BH, N]
+  const float* Ks;        // [BH, N]
+  const float* Vs;        // [BH, nG, D]
+  __half* O;              // [BH, N, D]  (debug: [128, D] tile)
+  const int32_t* head_sel;
+  int32_t* S_dump;        // debug only
+  uint8_t* P_dump;        // debug only
+  int N, nblk, npad;
+  int dbg_bh, dbg_qtile;  // debug only
+  float scale_log2;       // log2(e) / sqrt(D)
+};
+
+template <int D>
+struct SmemInt4 {
+  static constexpr int Q_BYTES = 128 * 128;
+  static constexpr int K_BYTES = 128 * 128;
+  static constexpr int V_BYTES = D * 128;
+  static constexpr int OFF_Q = 0;
+  static constexpr int OFF_K = OFF_Q + Q_BYTES;
+  static constexpr int OFF_V = OFF_K + KV_STAGES * K_BYTES;
+  static constexpr int OFF_KS = OFF_V + KV_STAGES * V_BYTES;          // float [2][128]
+  static constexpr int OFF_VS = OFF_KS + 2 * 128 * 4;                 // float [2][D]
+  static constexpr int OFF_AB = OFF_VS + 2 * D * 4;                   // float2 [AB_RING][128]
+  static constexpr int OFF_L = OFF_AB + AB_RING * 128 * 8;            // float [128]
+  static constexpr int OFF_BAR = OFF_L + 128 * 4;                     // mbarriers
+  static constexpr int NBAR = 1 + 4 * KV_STAGES + 2 + 2 + 2 + 2 + AB_RING + 1;
+  static constexpr int OFF_TMEM = OFF_BAR + NBAR * 8;
+  static constexpr int TOTAL = OFF_TMEM + 16 + 1024;                  // + alignment slack
+};
+
+__device__ __forceinline__ float ex2_approx(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
 }
-extern "C" int rotattn_fwd_int4_debug(const rotattn_params* p, const uint8_t*, const float*, const uint8_t*, const float*,
-                                      const uint8_t*, const float*, int32_t, int32_t, int32_t*, uint8_t*, void*, void*, size_t,
-                                      int32_t, void*) {
-  (void)p; return ROTATTN_ERR_UNSUPPORTED;
+
+template <int D, int P_MODE, int P_NORM, bool DEBUG>
+__global__ void __launch_bounds__(384, 1)
+fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
+                const __grid_constant__ CUtensorMap tmV, const FwdInt4Args a) {
+  using L = SmemInt4<D>;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  uint8_t* sQ = smem + L::OFF_Q;
+  uint8_t* sK = smem + L::OFF_K;
+  uint8_t* sV = smem + L::OFF_V;
+  float* sKs = (float*)(smem + L::OFF_KS);
+  float* sVs = (float*)(smem + L::OFF_VS);
+  float2* sAB = (float2*)(smem + L::OFF_AB);
+  float* sL = (float*)(smem + L::OFF_L);
+  uint64_t* bars = (uint64_t*)(smem + L::OFF_BAR);
+  uint64_t* q_full = bars;
+  uint64_t* k_full = q_full + 1;
+  uint64_t* k_empty = k_full + KV_STAGES;
+  uint64_t* v_full = k_empty + KV_STAGES;
+  uint64_t* v_empty = v_full + KV_STAGES;
+  uint64_t* s_full = v_empty + KV_STAGES;     // [2] MMA -> softmax
+  uint64_t* p_full = s_full + 2;              // [2] softmax -> MMA (count 128)
+  uint64_t* pv_full = p_full + 2;             // [2] MMA -> drain
+  uint64_t* pv_empty = pv_full + 2;           // [2] drain -> MMA (count 128)
+  uint64_t* ab_full = pv_empty + 2;           // [AB_RING] softmax -> drain (count 128)
+  uint64_t* l_full = ab_full + AB_RING;       // softmax -> drain (count 128)
+  uint32_t* tmem_slot = (uint32_t*)(smem + L::OFF_TMEM);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int qtile = DEBUG ? a.dbg_qtile : blockIdx.x;
+  const int bh = DEBUG ? a.dbg_bh : (a.head_sel ? a.head_sel[blockIdx.y] : (int)blockIdx.y);
+  const int q0 = qtile * kTile;
+  const int nblk = a.nblk;
+
+  if (threadIdx.x == 0) {
+    mbar_init(q_full, 1);
+    for (int i = 0; i < KV_STAGES; ++i) { mbar_init(&k_full[i], 1); mbar_init(&k_empty[i], 1); mbar_init(&v_full[i], 1); mbar_init(&v_empty[i], 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&s_full[i], 1); mbar_init(&p_full[i], 128); mbar_init(&pv_full[i], 1); mbar_init(&pv_empty[i], 128); }
+    for (int i = 0; i < AB_RING; ++i) mbar_init(&ab_full[i], 128);
+    mbar_init(l_full, 128);
+    fence_mbar_init();
+  }
+  if (warp == 2) tmem_alloc(tmem_slot, 512);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+  constexpr uint32_t TM_S = 0, TM_PV = 256;
+
+  if (warp < 4) {
+   asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+   if (warp == 0) {
+    // ------------------------------------------------------------------ TMA producer
+    if (lane == 0) {
+      tma_prefetch_desc(&tmQ); tma_prefetch_desc(&tmK); tma_prefetch_desc(&tmV);
+      mbar_arrive_expect_tx(q_full, L::Q_BYTES);
+      tma_load_3d(sQ, &tmQ, q_full, 0, q0, bh);
+      int s = 0; uint32_t ph = 0;
+      for (int j = 0; j < nblk; ++j) {
+        mbar_wait(&k_empty[s], ph ^ 1);
+        mbar_arrive_expect_tx(&k_full[s], L::K_BYTES);
+        tma_load_3d(sK + s * L::K_BYTES, &tmK, &k_full[s], 0, j * kTile, bh);
+        mbar_wait(&v_empty[s], ph ^ 1);
+        mbar_arrive_expect_tx(&v_full[s], L::V_BYTES);
+        tma_load_3d(sV + s * L::V_BYTES, &tmV, &v_full[s], j * kTile, 0, bh);
+        if (++s == KV_STAGES) { s = 0; ph ^= 1; }
+      }
+    }
+   } else if (warp == 1) {
+    // ------------------------------------------------------------------ MMA issuer
+    if (lane == 0) {
+      constexpr uint32_t idesc_s = umma_idesc(2, 1, 1, 128, 128);      // s32 <- s8 x s8
+      constexpr uint32_t idesc_pv = umma_idesc(2, 0, 1, 128, D);       // s32 <- u8 x s8
+      constexpr int KSTEPS_S = D / 32;                                 // D=64 rows are zero-padded to 128 B
+      const uint64_t qd = umma_desc_k128(smem_u32(sQ));
+      mbar_wait(q_full, 0);
+      mbar_wait(&k_full[0], 0);
+      tc_fence_after();
+      {
+        const uint64_t kd = umma_desc_k128(smem_u32(sK));
+#pragma unroll
+        for (int k = 0; k < KSTEPS_S; ++k) mma_ss<MmaKind::I8>(tmem_base + TM_S, qd + 2 * k, kd + 2 * k, idesc_s, k != 0);
+        tc_commit(&k_empty[0]);
+        tc_commit(&s_full[0]);
+      }
+      int ks = 1; uint32_t kph = 0;       // K ring position of block j+1
+      int vs = 0; uint32_t vph = 0;       // V ring position of block j
+      for (int j = 0; j < nblk; ++j) {
+        const int b = j & 1;
+        if (j + 1 < nblk) {
+          if (ks == KV_STAGES) { ks = 0; kph ^= 1; }
+          mbar_wait(&k_full[ks], kph);
+          tc_fence_after();
+          const uint64_t kd = umma_desc_k128(smem_u32(sK + ks * L::K_BYTES));
+#pragma unroll
+          for (int k = 0; k < KSTEPS_S; ++k)
+            mma_ss<MmaKind::I8>(tmem_base + TM_S + (b ^ 1) * 128, qd + 2 * k, kd + 2 * k, idesc_s, k != 0);
+          tc_commit(&k_empty[ks]);
+          tc_commit(&s_full[b ^ 1]);
+          ++ks;
+        }
+        mbar_wait(&p_full[b], (j >> 1) & 1);
+        mbar_wait(&v_full[vs], vph);
+        mbar_wait(&pv_empty[b], ((j >> 1) & 1) ^ 1);
+        tc_fence_after();
+        const uint64_t vd = umma_desc_k128(smem_u32(sV + vs * L::V_BYTES));
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+          mma_ts<MmaKind::I8>(tmem_base + TM_PV + b * 128, tmem_base + TM_S + b * 128 + 8 * k, vd + 2 * k, idesc_pv, k != 0);
+        tc_commit(&v_empty[vs]);
+        tc_commit(&pv_full[b]);
+        if (++vs == KV_STAGES) { vs = 0; vph ^= 1; }
+      }
+    }
+   }
+  } else if (warp < 8) {
+    // ------------------------------------------------------------------ softmax group (1 thread = 1 query row)
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 216;");
+    const int r = threadIdx.x - 128;
+    const int row = q0 + r;
+    const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
+    const float qs = (row < a.N) ? a.Qs[(size_t)bh * a.N + row] : 0.f;
+    const float* ksrc = a.Ks + (size_t)bh * a.N;
+    constexpr float LEVELS = P_MODE == ROTATTN_P_ASYM15 ? 15.f : 7.f;
+    float m_run = -INFINITY, l_run = 0.f;
+    sKs[r] = (r < a.N) ? ksrc[r] * a.scale_log2 : 0.f;
+    for (int j = 0; j < nblk; ++j) {
+      const int b = j & 1;
+      bar_sync(1, 128);                                  // ks'(j) visible; everyone is past block j-1
+      float ks_next = 0.f;
+      if (j + 1 < nblk) { int kj = (j + 1) * kTile + r; ks_next = (kj < a.N) ? ksrc[kj] * a.scale_log2 : 0.f; }
+      const float* ksb = sKs + b * 128;
+      const int nvalid = min(kTile, a.N - j * kTile);    // < 128 only on the ragged last block
+      mbar_wait(&s_full[b], (j >> 1) & 1);
+      tc_fence_after();
+      float t[128];
+      float tmax = -INFINITY;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        uint32_t v[32];
+        tmem_ld32(tmem_base + lane_off + TM_S + b * 128 + c * 32, v);
+        tmem_wait_ld();
+        if (DEBUG) {
+#pragma unroll
+          for (int i = 0; i < 32; ++i) a.S_dump[(size_t)r * a.npad + j * kTile + c * 32 + i] = (int32_t)v[i];
+        }
+#pragma unroll
+        for (int i = 0; i < 32; ++i) {
+          const float x = (float)(int32_t)v[i] * ksb[c * 32 + i];      // acc * Ks_j * log2e/sqrt(D)
+          t[c * 32 + i] = x;
+          if (c * 32 + i < nvalid) tmax = fmaxf(tmax, x);              // keys >= N are masked out of the max
+        }
+      }
+      // online softmax bookkeeping (log2 domain): mt = qs * tmax is the block row max of s*log2e
+      const float mt = qs * tmax;
+      const float m_new = fmaxf(m_run, mt);
+      const float ref = P_NORM == ROTATTN_NORM_ROWBLOCK ? mt : m_new;
+      const float alpha = ex2_approx(m_run - m_new);                   // first block: exp2(-inf) = 0
+      const float beta = P_NORM == ROTATTN_NORM_ROWBLOCK ? ex2_approx(mt - m_new) : 1.f;
+      float lsum = 0.f;
+      uint32_t pw[32];
+#pragma unroll
+      for (int g = 0; g < 32; ++g) {
+        uint32_t fb[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const int col = g * 4 + i;
+          float e = fmaf(t[col], qs, -ref);
+          if (col >= nvalid) e = -INFINITY;
+          const float p = ex2_approx(e);
+          lsum += p;
+          fb[i] = __float_as_uint(fmaf(p, LEVELS, 12582912.f));        // low byte = rne(LEVELS * p)
+        }
+        const uint32_t lo = __byte_perm(fb[0], fb[1], 0x0040);
+        const uint32_t hi = __byte_perm(fb[2], fb[3], 0x0040);
+        pw[g] = __byte_perm(lo, hi, 0x5410);
+      }
+      if (DEBUG) {
+#pragma unroll
+        for (int g = 0; g < 32; ++g) *reinterpret_cast<uint32_t*>(a.P_dump + (size_t)r * a.npad + j * kTile + g * 4) = pw[g];
+      }
+      tmem_st32(tmem_base + lane_off + TM_S + b * 128, pw);            // u8 P tile aliases S columns [0,32)
+      sAB[(j % AB_RING) * 128 + r] = make_float2(alpha, beta * (1.f / LEVELS));
+      l_run = alpha * l_run + beta * lsum;
+      m_run = m_new;
+      tmem_wait_st();
+      tc_fence_before();
+      mbar_arrive(&p_full[b]);
+      mbar_arrive(&ab_full[j % AB_RING]);
+      if (j + 1 < nblk) sKs[(b ^ 1) * 128 + r] = ks_next;
+    }
+    sL[r] = l_run;
+    mbar_arrive(l_full);
+  } else {
+    // ------------------------------------------------------------------ drain group (1 thread = 1 query row of O)
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 216;");
+    const int r = threadIdx.x - 256;
+    const int row = q0 + r;
+    const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
+    const float* vsrc = a.Vs + (size_t)bh * nblk * D;
+    float o[D];
+#pragma unroll
+    for (int d = 0; d < D; ++d) o[d] = 0.f;
+    if (r < D) sVs[r] = vsrc[r];
+    for (int j = 0; j < nblk; ++j) {
+      const int b = j & 1;
+      bar_sync(2, 128);
+      float vs_next = 0.f;
+      if (j + 1 < nblk && r < D) vs_next = vsrc[(size_t)(j + 1) * D + r];
+      const float* vsb = sVs + b * D;
+      mbar_wait(&ab_full[j % AB_RING], (j / AB_RING) & 1);
+      const float2 ab = sAB[(j % AB_RING) * 128 + r];
+      mbar_wait(&pv_full[b], (j >> 1) & 1);
+      tc_fence_after();
+#pragma unroll
+      for (int c = 0; c < D / 32; ++c) {
+        uint32_t v[32];
+        tmem_ld32(tmem_base + lane_off + TM_PV + b * 128 + c * 32, v);
+        tmem_wait_ld();
+#pragma unroll
+        for (int i = 0; i < 32; ++i) {
+          const float y = (float)(int32_t)v[i] * vsb[c * 32 + i];      // pv * Vs[g][d]
+          o[c * 32 + i] = fmaf(o[c * 32 + i], ab.x, ab.y * y);         // O = alpha O + (beta/levels) * y
+        }
+      }
+      tc_fence_before();
+      mbar_arrive(&pv_empty[b]);
+      if (j + 1 < nblk && r < D) sVs[(b ^ 1) * D + r] = vs_next;
+    }
+    mbar_wait(l_full, 0);
+    const float inv_l = 1.f / sL[r];
+    if (row < a.N) {
+      __half* dst = DEBUG ? a.O + (size_t)r * D : a.O + ((size_t)bh * a.N + row) * D;
+#pragma unroll
+      for (int d = 0; d < D; d += 8) {
+        __half2 h[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) h[i] = __floats2half2_rn(o[d + 2 * i] * inv_l, o[d + 2 * i + 1] * inv_l);
+        *reinterpret_cast<uint4*>(dst + d) = *reinterpret_cast<uint4*>(h);
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 2) tmem_dealloc(tmem_base, 512);
+}
+
+}  // namespace rotattn
+
+using namespace rotattn;
+
+namespace {
+
+template <int D, bool DEBUG>
+int launch_variant(const rotattn_params& p, const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv,
+                   const FwdInt4Args& a, dim3 grid, cudaStream_t cs) {
+  constexpr int smem = SmemInt4<D>::TOTAL;
+#define ROTATTN_LAUNCH(PM, PN)                                                                                      \
+  do {                                                                                                              \
+    ROTATTN_CUDA_TRY(cudaFuncSetAttribute(fwd_int4_kernel<D, PM, PN, DEBUG>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); \
+    fwd_int4_kernel<D, PM, PN, DEBUG><<<grid, 384, smem, cs>>>(tq, tk, tv, a);                                      \
+  } while (0)
+  if (p.p_mode == ROTATTN_P_ASYM15 && p.p_norm == ROTATTN_NORM_ROWBLOCK) ROTATTN_LAUNCH(ROTATTN_P_ASYM15, ROTATTN_NORM_ROWBLOCK);
+  else if (p.p_mode == ROTATTN_P_ASYM15) ROTATTN_LAUNCH(ROTATTN_P_ASYM15, ROTATTN_NORM_RUNNING);
+  else if (p.p_norm == ROTATTN_NORM_ROWBLOCK) ROTATTN_LAUNCH(ROTATTN_P_SYM7, ROTATTN_NORM_ROWBLOCK);
+  else ROTATTN_LAUNCH(ROTATTN_P_SYM7, ROTATTN_NORM_RUNNING);
+#undef ROTATTN_LAUNCH
+  ROTATTN_CUDA_TRY(cudaGetLastError());
+  return ROTATTN_OK;
+}
+
+int fwd_int4_common(const rotattn_params* p, const uint8_t* Q4, const float* Qs, const uint8_t* K4, const float* Ks,
+                    const uint8_t* V4, const float* Vs, void* O, const int32_t* head_sel, int32_t n_sel,
+                    void* workspace, size_t ws_bytes, int32_t ws_state, void* stream,
+                    bool debug, int32_t bh, int32_t q_tile, int32_t* S_dump, uint8_t* P_dump) {
+  int st = rotattn_validate(p);
+  if (st != ROTATTN_OK) return st;
+  if (!Q4 || !Qs || !K4 || !Ks || !V4 || !Vs || !O || !workspace) return ROTATTN_ERR_INVALID_ARG;
+  const int BH = p->B * p->H;
+  const int nblk = ceil_div(p->N, kTile);
+  if (head_sel && (n_sel < 1 || n_sel > BH)) return ROTATTN_ERR_INVALID_ARG;
+  if (debug && (bh < 0 || bh >= BH || q_tile < 0 || q_tile >= nblk || !S_dump || !P_dump)) return ROTATTN_ERR_INVALID_ARG;
+  WsInt4 ws(*p);
+  if (ws_bytes < ws.total) return ROTATTN_ERR_WORKSPACE_TOO_SMALL;
+  if ((st = check_device_sm100()) != ROTATTN_OK) return st;
+  cudaStream_t cs = (cudaStream_t)stream;
+  int8_t* q8 = (int8_t*)workspace + ws.q8;
+  int8_t* k8 = (int8_t*)workspace + ws.k8;
+  int8_t* v8t = (int8_t*)workspace + ws.v8t;
+  if (!(ws_state & ROTATTN_WS_HAS_QK)) {
+    if ((st = launch_unpack_qk(*p, Q4, q8, cs)) != ROTATTN_OK) return st;
+    if ((st = launch_unpack_qk(*p, K4, k8, cs)) != ROTATTN_OK) return st;
+  }
+  if (!(ws_state & ROTATTN_WS_HAS_V)) {
+    if ((st = launch_unpack_vt(*p, V4, v8t, ws.npad, cs)) != ROTATTN_OK) return st;
+  }
+  CUtensorMap tq, tk, tv;
+  const uint64_t N = p->N, D = p->D;
+  if ((st = make_tmap_3d(&tq, q8, 1, kQKRowBytes, N, BH, kQKRowBytes, N * kQKRowBytes, 128, 128)) != ROTATTN_OK) return st;
+  if ((st = make_tmap_3d(&tk, k8, 1, kQKRowBytes, N, BH, kQKRowBytes, N * kQKRowBytes, 128, 128)) != ROTATTN_OK) return st;
+  if ((st = make_tmap_3d(&tv, v8t, 1, ws.npad, D, BH, ws.npad, D * ws.npad, 128, (uint32_t)D)) != ROTATTN_OK) return st;
+  FwdInt4Args a{};
+  a.Qs = Qs; a.Ks = Ks; a.Vs = Vs; a.O = (__half*)O; a.head_sel = head_sel;
+  a.S_dump = S_dump; a.P_dump = P_dump;
+  a.N = p->N; a.nblk = nblk; a.npad = ws.npad; a.dbg_bh = bh; a.dbg_qtile = q_tile;
+  a.scale_log2 = (float)(1.4426950408889634 / std::sqrt((double)p->D));
+  dim3 grid(debug ? 1 : nblk, debug ? 1 : (head_sel ? n_sel : BH));
+  if (p->D == 128) return debug ? launch_variant<128, true>(*p, tq, tk, tv, a, grid, cs) : launch_variant<128, false>(*p, tq, tk, tv, a, grid, cs);
+  return debug ? launch_variant<64, true>(*p, tq, tk, tv, a, grid, cs) : launch_variant<64, false>(*p, tq, tk, tv, a, grid, cs);
+}
+
+}  // namespace
+
+extern "C" int rotattn_fwd_int4(const rotattn_params* p, const uint8_t* Q4, const float* Qs, const uint8_t* K4,
+                                const float* Ks, const uint8_t* V4, const float* Vs, void* O, const int32_t* head_sel,
+                                int32_t n_sel, void* workspace, size_t ws_bytes, int32_t ws_state, void* stream) {
+  return fwd_int4_common(p, Q4, Qs, K4, Ks, V4, Vs, O, head_sel, n_sel, workspace, ws_bytes, ws_state, stream,
+                         false, 0, 0, nullptr, nullptr);
+}
+
+extern "C" int rotattn_fwd_int4_debug(const rotattn_params* p, const uint8_t* Q4, const float* Qs, const uint8_t* K4,
+                                      const float* Ks, const uint8_t* V4, const float* Vs, int32_t bh, int32_t q_tile,
+                                      int32_t* S_dump, uint8_t* P_dump, void* O_tile, void* workspace, size_t ws_bytes,
+                                      int32_t ws_state, void* stream) {
+  return fwd_int4_common(p, Q4, Qs, K4, Ks, V4, Vs, O_tile, nullptr, 0, workspace, ws_bytes, ws_state, stream,
+                         true, bh, q_tile, S_dump, P_dump);
 }
