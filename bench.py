@@ -49,7 +49,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(['nvidia-smi', '-i', str(self.index), f'--query-gpu={self.Q}',
-                                          '--format=csv,noheader,nounits', '-lms', '100'],
+                                          '--format=csv,noheader,nounits', '-lms', '20'],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -239,9 +239,10 @@ def main():
     int8_peak = 2.0 * pk['bf16']      # dense int8 = 2x bf16 nominal ratio (4.5 / 2.25 PFLOP/s) applied to the measured bf16 peak
     achieved = ops / (t_int4 * 1e-3) / 1e12
     traffic = None
-    tpath = os.path.join(ROOT, 'profiles', 'fwd_int4_traffic.json')
+    tpath = os.path.join(ROOT, 'profiles', 'fwd_int4_traffic.csv')     # dram__bytes_read+write of one ncu --set full capture
     if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get('dram_bytes_per_launch')
+        last = open(tpath).read().strip().splitlines()[-1].split(',')
+        traffic = int(last[-2]) if last[-2].isdigit() else None
     out = {
         'metric': METRIC, 'value': world * ops / (ms_step * 1e-3) / 1e12, 'unit': 'TOPS', 'n_gpus': world, 'steps': K, 'warmup': W,
         'ms_per_step': ms_step, 'higher_is_better': True, 'scaling': 'weak', 'vs_baseline': None, 'dtype': 'int8 codes (INT4 values) / int32 accumulate / fp32 softmax',
