@@ -1,40 +1,31 @@
-// rotattn_fwd_int4 (steps a4-a9): INT4 FlashAttention forward on tcgen05 kind::i8.
+// rotattn_fwd_int4 (steps a4-a9): INT4 FlashAttention forward on tcgen05 kind::i8, row-block P normaliser.
 //
 // One CTA = one 128-row query tile of one (b,h); 20 warps, warp-specialised:
 //   warp 0        TMA producer : Q tile once, K / V^T tiles through 3-stage shared-memory rings
 //   warp 1        MMA issuer   : S = Q K^T (int8 x int8 -> int32, TMEM), P~V (u8 from TMEM x int8 -> int32, TMEM)
-//   warp 2        TMEM allocator
-//   warps 4-11    softmax      : 2 threads per query row (64 keys each): int32 S -> dequant -> block row max ->
-//                                P^ = exp2 -> codes u = rne(15 P^) -> u8 P tile in TMEM
-//   warps 12-19   drain        : 2 threads per query row (D/2 channels each): int32 P~V block -> fp32 O registers
-//                                (alpha, beta, V scales), epilogue O/l
-// TMEM (512 columns): S[2] at 0/128 (the u8 P tile aliases the first 32 columns of its S buffer), PV[2] at 256/384.
+//   warp 2        TMEM allocator, then V-scale loader (Vs[g][:] -> shared ring)
+//   warp 3        K-scale loader (Ks[j] * log2e/sqrt(D) -> shared ring)
+//   warps 4-7     softmax group A: even KV blocks, one thread per query row
+//   warps 8-11    softmax group B: odd KV blocks
+//   warps 12-19   drain: 2 threads per query row (D/2 channels each): online-softmax bookkeeping (m, l, alpha, beta),
+//                 int32 P~V block -> fp32 O registers, epilogue O/l
+// With the row-block normaliser (reading 13) the codes of block j depend only on block j, so the two softmax
+// groups work on different blocks out of phase (one in its ALU phase while the other keeps the MUFU pipe busy) and
+// the running max lives in the drain threads.  Each softmax thread makes two passes over its S row in tensor memory
+// (pass 1: block row max, pass 2: exp2 / codes) in 32-column chunks, so it needs no 128-register row buffer.
+// TMEM (512 columns): S[2] at 0/128 (u8 P tile aliases the first 32 columns of its S buffer), PV[2] at 256/384.
 // The per-block drain is forced by the method: beta (row, block) and Vs (channel, block) change every KV block
 // (PAPER.md:L157 online softmax, L190 per-group V scales), so integer P~V cannot accumulate across blocks.
-// Two threads per row double the warps per scheduler (latency hiding) and halve the per-thread register tile;
-// packed fp32x2 arithmetic (FMUL2/FFMA2/FADD2) and 3-input max halve the issue slots of the element-wise work.
 #include <cmath>
 #include <cstdio>
-#include "tc_common.cuh"
+#include "fwd_int4.cuh"
 
 namespace rotattn {
 
 constexpr int KV_STAGES = 3;
 constexpr int AB_RING = 4;
-constexpr int kInt4Threads = 640;
-
-struct FwdInt4Args {
-  const float* Qs;        // [BH, N]
-  const float* Ks;        // [BH, N]
-  const float* Vs;        // [BH, nG, D]
-  __half* O;              // [BH, N, D]  (debug: [128, D] tile)
-  const int32_t* head_sel;
-  int32_t* S_dump;        // debug only
-  uint8_t* P_dump;        // debug only
-  int N, nblk, npad;
-  int dbg_bh, dbg_qtile;  // debug only
-  float scale_log2;       // log2(e) / sqrt(D)
-};
+constexpr int KS_RING = 4;
+constexpr int VS_RING = 4;
 
 template <int D>
 struct SmemInt4 {
@@ -44,50 +35,87 @@ struct SmemInt4 {
   static constexpr int OFF_Q = 0;
   static constexpr int OFF_K = OFF_Q + Q_BYTES;
   static constexpr int OFF_V = OFF_K + KV_STAGES * K_BYTES;
-  static constexpr int OFF_KS = OFF_V + KV_STAGES * V_BYTES;          // float [2][128]
-  static constexpr int OFF_VS = OFF_KS + 2 * 128 * 4;                 // float [2][D]
-  static constexpr int OFF_AB = OFF_VS + 2 * D * 4;                   // float2 [AB_RING][128]
-  static constexpr int OFF_MX = OFF_AB + AB_RING * 128 * 8;           // float [2 parity][2 halves][128]
-  static constexpr int OFF_L = OFF_MX + 2 * 2 * 128 * 4;              // float [2 halves][128]
-  static constexpr int OFF_BAR = OFF_L + 2 * 128 * 4;                 // mbarriers
-  static constexpr int NBAR = 1 + 4 * KV_STAGES + 2 + 2 + 2 + 2 + AB_RING + 1;
+  static constexpr int OFF_KS = OFF_V + KV_STAGES * V_BYTES;          // float [KS_RING][128]
+  static constexpr int OFF_VS = OFF_KS + KS_RING * 128 * 4;           // float [VS_RING][D]
+  static constexpr int OFF_AB = OFF_VS + VS_RING * D * 4;             // float2 [AB_RING][128]  (block max, block sum)
+  static constexpr int OFF_BAR = OFF_AB + AB_RING * 128 * 8;          // mbarriers
+  static constexpr int NBAR = 1 + 4 * KV_STAGES + 2 + 2 + 2 + 2 + AB_RING + 2 * KS_RING + 2 * VS_RING;
   static constexpr int OFF_TMEM = OFF_BAR + NBAR * 8;
-  static constexpr int TOTAL = OFF_TMEM + 16 + 1024;                  // + alignment slack
+  static constexpr int TOTAL = OFF_TMEM + 16;
 };
 
-__device__ __forceinline__ float ex2_approx(float x) {
-  float y;
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
+// ---- per-chunk element-wise work of the softmax threads (32 S columns of one query row) -------------------------
+// t = acc * Ks_j * log2e/sqrt(D) (the query scale Qs_i > 0 is applied after the max); keys >= N are masked to -inf.
+template <bool MASK>
+__device__ __forceinline__ void chunk_scale(const uint32_t (&v)[32], const float2* ks2, int nvalid_rel, float2 (&t2)[16]) {
+#pragma unroll
+  for (int i = 0; i < 16; ++i) {
+    t2[i] = fmul2(make_float2((float)(int32_t)v[2 * i], (float)(int32_t)v[2 * i + 1]), ks2[i]);
+    if (MASK) {
+      if (2 * i >= nvalid_rel) t2[i].x = -INFINITY;
+      if (2 * i + 1 >= nvalid_rel) t2[i].y = -INFINITY;
+    }
+  }
 }
 
-template <int D, int P_MODE, int P_NORM, bool DEBUG>
+template <bool MASK>
+__device__ __forceinline__ void chunk_max(const uint32_t (&v)[32], const float2* ks2, int nvalid_rel, float& mx0, float& mx1) {
+  float2 t2[16];
+  chunk_scale<MASK>(v, ks2, nvalid_rel, t2);
+#pragma unroll
+  for (int i = 0; i < 16; i += 2) { mx0 = fmax3(mx0, t2[i].x, t2[i].y); mx1 = fmax3(mx1, t2[i + 1].x, t2[i + 1].y); }
+}
+
+// P^ = exp2(t * Qs_i - mt); codes u = rne(LEVELS * P^) taken from the low byte of fma(P^, LEVELS, 1.5 * 2^23)
+// (Eq.12 L166-168 with the fixed scale 15 / Eq.11 L161 with 7); four codes per 32-bit TMEM column.
+template <bool MASK, int P_MODE>
+__device__ __forceinline__ void chunk_exp(const uint32_t (&v)[32], const float2* ks2, int nvalid_rel, float2 qs2, float2 nref2,
+                                          float2& ls0, float2& ls1, uint32_t (&pw)[8]) {
+  constexpr float LEVELS = P_MODE == ROTATTN_P_ASYM15 ? 15.f : 7.f;
+  const float2 lev2 = make_float2(LEVELS, LEVELS), magic2 = make_float2(12582912.f, 12582912.f);
+  float2 t2[16];
+  chunk_scale<MASK>(v, ks2, nvalid_rel, t2);
+#pragma unroll
+  for (int g = 0; g < 8; ++g) {
+    const float2 e0 = ffma2(t2[2 * g], qs2, nref2), e1 = ffma2(t2[2 * g + 1], qs2, nref2);
+    const float2 p0 = make_float2(ex2_approx(e0.x), ex2_approx(e0.y));
+    const float2 p1 = make_float2(ex2_approx(e1.x), ex2_approx(e1.y));
+    ls0 = fadd2(ls0, p0);
+    ls1 = fadd2(ls1, p1);
+    const float2 f0 = ffma2(p0, lev2, magic2), f1 = ffma2(p1, lev2, magic2);
+    const uint32_t lo = __byte_perm(__float_as_uint(f0.x), __float_as_uint(f0.y), 0x0040);
+    const uint32_t hi = __byte_perm(__float_as_uint(f1.x), __float_as_uint(f1.y), 0x0040);
+    pw[g] = __byte_perm(lo, hi, 0x5410);
+  }
+}
+
+template <int D, int P_MODE, bool DEBUG>
 __global__ void __launch_bounds__(kInt4Threads, 1)
 fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                 const __grid_constant__ CUtensorMap tmV, const FwdInt4Args a) {
   using L = SmemInt4<D>;
-  extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  extern __shared__ __align__(1024) uint8_t smem[];      // no static shared memory in this kernel: base is 1024-aligned
   uint8_t* sQ = smem + L::OFF_Q;
   uint8_t* sK = smem + L::OFF_K;
   uint8_t* sV = smem + L::OFF_V;
   float* sKs = (float*)(smem + L::OFF_KS);
   float* sVs = (float*)(smem + L::OFF_VS);
   float2* sAB = (float2*)(smem + L::OFF_AB);
-  float* sMx = (float*)(smem + L::OFF_MX);
-  float* sL = (float*)(smem + L::OFF_L);
   uint64_t* bars = (uint64_t*)(smem + L::OFF_BAR);
   uint64_t* q_full = bars;
   uint64_t* k_full = q_full + 1;
   uint64_t* k_empty = k_full + KV_STAGES;
   uint64_t* v_full = k_empty + KV_STAGES;
   uint64_t* v_empty = v_full + KV_STAGES;
-  uint64_t* s_full = v_empty + KV_STAGES;     // [2] MMA -> softmax
-  uint64_t* p_full = s_full + 2;              // [2] softmax -> MMA (count 256)
+  uint64_t* s_full = v_empty + KV_STAGES;     // [2] MMA -> softmax group (buffer b belongs to group b)
+  uint64_t* p_full = s_full + 2;              // [2] softmax group -> MMA (count 128)
   uint64_t* pv_full = p_full + 2;             // [2] MMA -> drain
   uint64_t* pv_empty = pv_full + 2;           // [2] drain -> MMA (count 256)
-  uint64_t* ab_full = pv_empty + 2;           // [AB_RING] softmax (half 0) -> drain (count 128)
-  uint64_t* l_full = ab_full + AB_RING;       // softmax -> drain (count 256)
+  uint64_t* ab_full = pv_empty + 2;           // [AB_RING] softmax -> drain (count 128)
+  uint64_t* ks_full = ab_full + AB_RING;      // [KS_RING] loader -> softmax (count 32)
+  uint64_t* ks_empty = ks_full + KS_RING;     // [KS_RING] softmax -> loader (count 128)
+  uint64_t* vs_full = ks_empty + KS_RING;     // [VS_RING] loader -> drain (count 32)
+  uint64_t* vs_empty = vs_full + VS_RING;     // [VS_RING] drain -> loader (count 256)
   uint32_t* tmem_slot = (uint32_t*)(smem + L::OFF_TMEM);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -97,11 +125,13 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   const int nblk = a.nblk;
 
   if (threadIdx.x == 0) {
+    if (smem_u32(smem) & 1023u) __trap();     // SWIZZLE_128B operand tiles need 1024-byte alignment
     mbar_init(q_full, 1);
     for (int i = 0; i < KV_STAGES; ++i) { mbar_init(&k_full[i], 1); mbar_init(&k_empty[i], 1); mbar_init(&v_full[i], 1); mbar_init(&v_empty[i], 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(&s_full[i], 1); mbar_init(&p_full[i], 256); mbar_init(&pv_full[i], 1); mbar_init(&pv_empty[i], 256); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&s_full[i], 1); mbar_init(&p_full[i], 128); mbar_init(&pv_full[i], 1); mbar_init(&pv_empty[i], 256); }
     for (int i = 0; i < AB_RING; ++i) mbar_init(&ab_full[i], 128);
-    mbar_init(l_full, 256);
+    for (int i = 0; i < KS_RING; ++i) { mbar_init(&ks_full[i], 32); mbar_init(&ks_empty[i], 128); }
+    for (int i = 0; i < VS_RING; ++i) { mbar_init(&vs_full[i], 32); mbar_init(&vs_empty[i], 256); }
     fence_mbar_init();
   }
   if (warp == 2) tmem_alloc(tmem_slot, 512);
@@ -111,7 +141,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   const uint32_t tmem_base = *tmem_slot;
   constexpr uint32_t TM_S = 0, TM_PV = 256;
 
-  // register pool of the CTA = 640 x 96; after redistribution 128 x 32 + 256 x 104 + 256 x 120 = 61440 (must not exceed it)
+  // register pool of the CTA = 640 x 96; after redistribution 128 x 32 + 256 x 96 + 256 x 120 = 59392 (must not exceed it)
   if (warp < 4) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");
     if (warp == 0) {
@@ -138,168 +168,152 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         constexpr uint32_t idesc_pv = umma_idesc(2, 0, 1, 128, D);       // s32 <- u8 x s8
         constexpr int KSTEPS_S = D / 32;                                 // D=64 rows are zero-padded to 128 B
         const uint64_t qd = umma_desc_k128(smem_u32(sQ));
-        mbar_wait(q_full, 0);
-        mbar_wait(&k_full[0], 0);
-        tc_fence_after();
-        {
-          const uint64_t kd = umma_desc_k128(smem_u32(sK));
+        auto issue_s = [&](int m) {                                      // S(m) -> buffer m & 1
+          const int st = m % KV_STAGES;
+          mbar_wait(&k_full[st], (m / KV_STAGES) & 1);
+          tc_fence_after();
+          const uint64_t kd = umma_desc_k128(smem_u32(sK + st * L::K_BYTES));
 #pragma unroll
-          for (int k = 0; k < KSTEPS_S; ++k) mma_ss<MmaKind::I8>(tmem_base + TM_S, qd + 2 * k, kd + 2 * k, idesc_s, k != 0);
-          tc_commit(&k_empty[0]);
-          tc_commit(&s_full[0]);
-        }
-        int ks = 1; uint32_t kph = 0;       // K ring position of block j+1
-        int vs = 0; uint32_t vph = 0;       // V ring position of block j
+          for (int k = 0; k < KSTEPS_S; ++k)
+            mma_ss<MmaKind::I8>(tmem_base + TM_S + (m & 1) * 128, qd + 2 * k, kd + 2 * k, idesc_s, k != 0);
+          tc_commit(&k_empty[st]);
+          tc_commit(&s_full[m & 1]);
+        };
+        mbar_wait(q_full, 0);
+        issue_s(0);
+        if (nblk > 1) issue_s(1);
         for (int j = 0; j < nblk; ++j) {
           const int b = j & 1;
-          if (j + 1 < nblk) {
-            if (ks == KV_STAGES) { ks = 0; kph ^= 1; }
-            mbar_wait(&k_full[ks], kph);
-            tc_fence_after();
-            const uint64_t kd = umma_desc_k128(smem_u32(sK + ks * L::K_BYTES));
-#pragma unroll
-            for (int k = 0; k < KSTEPS_S; ++k)
-              mma_ss<MmaKind::I8>(tmem_base + TM_S + (b ^ 1) * 128, qd + 2 * k, kd + 2 * k, idesc_s, k != 0);
-            tc_commit(&k_empty[ks]);
-            tc_commit(&s_full[b ^ 1]);
-            ++ks;
-          }
+          const int vst = j % KV_STAGES;
           mbar_wait(&p_full[b], (j >> 1) & 1);
-          mbar_wait(&v_full[vs], vph);
+          mbar_wait(&v_full[vst], (j / KV_STAGES) & 1);
           mbar_wait(&pv_empty[b], ((j >> 1) & 1) ^ 1);
           tc_fence_after();
-          const uint64_t vd = umma_desc_k128(smem_u32(sV + vs * L::V_BYTES));
+          const uint64_t vd = umma_desc_k128(smem_u32(sV + vst * L::V_BYTES));
 #pragma unroll
           for (int k = 0; k < 4; ++k)
             mma_ts<MmaKind::I8>(tmem_base + TM_PV + b * 128, tmem_base + TM_S + b * 128 + 8 * k, vd + 2 * k, idesc_pv, k != 0);
-          tc_commit(&v_empty[vs]);
+          tc_commit(&v_empty[vst]);
           tc_commit(&pv_full[b]);
-          if (++vs == KV_STAGES) { vs = 0; vph ^= 1; }
+          if (j + 2 < nblk) issue_s(j + 2);                              // reuses S buffer b after P(j) was consumed
         }
+      }
+    } else if (warp == 2) {
+      // ---------------------------------------------------------------- V-scale loader
+      const float* vsrc = a.Vs + (size_t)bh * nblk * D;
+      for (int j = 0; j < nblk; ++j) {
+        const int s = j % VS_RING;
+        mbar_wait(&vs_empty[s], ((j / VS_RING) & 1) ^ 1);
+#pragma unroll
+        for (int i = 0; i < D / 32; ++i) sVs[s * D + i * 32 + lane] = vsrc[(size_t)j * D + i * 32 + lane];
+        mbar_arrive(&vs_full[s]);
+      }
+    } else {
+      // ---------------------------------------------------------------- K-scale loader: Ks_j * log2e/sqrt(D)
+      const float* ksrc = a.Ks + (size_t)bh * a.N;
+      for (int j = 0; j < nblk; ++j) {
+        const int s = j % KS_RING;
+        mbar_wait(&ks_empty[s], ((j / KS_RING) & 1) ^ 1);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const int kj = j * kTile + i * 32 + lane;
+          sKs[s * 128 + i * 32 + lane] = (kj < a.N) ? ksrc[kj] * a.scale_log2 : 0.f;
+        }
+        mbar_arrive(&ks_full[s]);
       }
     }
   } else if (warp < 12) {
-    // ------------------------------------------------------------------ softmax: 2 threads per query row
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 104;");
-    const int tsm = threadIdx.x - 128;
-    const int h = tsm >> 7, r = tsm & 127;          // h: which 64-key half of the block this thread owns
-    const int cb = 64 * h;
+    // ------------------------------------------------------------------ softmax groups: A = even blocks, B = odd blocks
+    const int g = (warp - 4) >> 2;                   // group index = S buffer index
+    const int r = (threadIdx.x - 128) & 127;
     const int row = q0 + r;
     const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
     // qs >= 1e-30 keeps (-inf) * qs well defined for masked keys; an all-zero query row still gives s == 0 everywhere
     const float qs = (row < a.N) ? fmaxf(a.Qs[(size_t)bh * a.N + row], 1e-30f) : 1e-30f;
     const float2 qs2 = make_float2(qs, qs);
-    const float* ksrc = a.Ks + (size_t)bh * a.N;
-    constexpr float LEVELS = P_MODE == ROTATTN_P_ASYM15 ? 15.f : 7.f;
-    const float2 lev2 = make_float2(LEVELS, LEVELS), magic2 = make_float2(12582912.f, 12582912.f);
-    float m_run = -INFINITY, l_run = 0.f;
-    if (h == 0) sKs[r] = (r < a.N) ? ksrc[r] * a.scale_log2 : 0.f;
-    for (int j = 0; j < nblk; ++j) {
-      const int b = j & 1;
-      bar_sync(1, 256);                                  // ks'(j) visible; everyone is past block j-1
-      float ks_next = 0.f;
-      if (h == 0 && j + 1 < nblk) { int kj = (j + 1) * kTile + r; ks_next = (kj < a.N) ? ksrc[kj] * a.scale_log2 : 0.f; }
-      const float2* ksb2 = reinterpret_cast<const float2*>(sKs + b * 128 + cb);
+    const uint32_t s_addr = tmem_base + lane_off + TM_S + g * 128;
+    for (int j = g; j < nblk; j += 2) {
+      const int ring = j % KS_RING;
+      const float2* ks2 = reinterpret_cast<const float2*>(sKs + ring * 128);
       const int nvalid = min(kTile, a.N - j * kTile);    // < 128 only on the ragged last block
-      mbar_wait(&s_full[b], (j >> 1) & 1);
+      const bool ragged = nvalid < kTile;
+      mbar_wait(&ks_full[ring], (j / KS_RING) & 1);
+      mbar_wait(&s_full[g], (j >> 1) & 1);
       tc_fence_after();
-      float2 t2[32];
-      {
-        uint32_t v0[32], v1[32];
-        tmem_ld32(tmem_base + lane_off + TM_S + b * 128 + cb, v0);
-        tmem_ld32(tmem_base + lane_off + TM_S + b * 128 + cb + 32, v1);
+      uint32_t va[32], vb[32];
+      // ---- pass 1: block row max
+      float mx0 = -INFINITY, mx1 = -INFINITY;
+      tmem_ld32(s_addr, va);
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
         tmem_wait_ld();
+        uint32_t(&cur)[32] = (c & 1) ? vb : va;
+        uint32_t(&nxt)[32] = (c & 1) ? va : vb;
+        tmem_ld32(s_addr + ((c + 1) & 3) * 32, nxt);     // chunk c+1 (after chunk 3: chunk 0 again, for pass 2)
+        if (ragged) chunk_max<true>(cur, ks2 + c * 16, nvalid - c * 32, mx0, mx1);
+        else chunk_max<false>(cur, ks2 + c * 16, 32, mx0, mx1);
+      }
+      const float mt = qs * fmaxf(mx0, mx1);             // block row max of s * log2e
+      const float2 nref2 = make_float2(-mt, -mt);
+      // ---- pass 2: P^, row sum, codes -> u8 P tile (aliases S columns [0,32) of this buffer)
+      float2 ls0 = make_float2(0.f, 0.f), ls1 = make_float2(0.f, 0.f);
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        tmem_wait_ld();
+        uint32_t(&cur)[32] = (c & 1) ? vb : va;
+        uint32_t(&nxt)[32] = (c & 1) ? va : vb;
+        if (c < 3) tmem_ld32(s_addr + (c + 1) * 32, nxt);
         if (DEBUG) {
 #pragma unroll
-          for (int i = 0; i < 32; ++i) {
-            a.S_dump[(size_t)r * a.npad + j * kTile + cb + i] = (int32_t)v0[i];
-            a.S_dump[(size_t)r * a.npad + j * kTile + cb + 32 + i] = (int32_t)v1[i];
-          }
+          for (int i = 0; i < 32; ++i) a.S_dump[(size_t)r * a.npad + j * kTile + c * 32 + i] = (int32_t)cur[i];
         }
+        uint32_t pw[8];
+        if (ragged) chunk_exp<true, P_MODE>(cur, ks2 + c * 16, nvalid - c * 32, qs2, nref2, ls0, ls1, pw);
+        else chunk_exp<false, P_MODE>(cur, ks2 + c * 16, 32, qs2, nref2, ls0, ls1, pw);
+        if (DEBUG) {
 #pragma unroll
-        for (int i = 0; i < 16; ++i) {                                 // t = acc * Ks_j * log2e/sqrt(D)
-          t2[i] = fmul2(make_float2((float)(int32_t)v0[2 * i], (float)(int32_t)v0[2 * i + 1]), ksb2[i]);
-          t2[16 + i] = fmul2(make_float2((float)(int32_t)v1[2 * i], (float)(int32_t)v1[2 * i + 1]), ksb2[16 + i]);
+          for (int q = 0; q < 8; ++q) *reinterpret_cast<uint32_t*>(a.P_dump + (size_t)r * a.npad + j * kTile + c * 32 + q * 4) = pw[q];
         }
+        tmem_st8(s_addr + c * 8, pw);
       }
-      if (nvalid < kTile) {                                            // keys >= N: masked out of max, sum and codes
-#pragma unroll
-        for (int i = 0; i < 32; ++i) {
-          if (cb + 2 * i >= nvalid) t2[i].x = -INFINITY;
-          if (cb + 2 * i + 1 >= nvalid) t2[i].y = -INFINITY;
-        }
-      }
-      float mx0 = -INFINITY, mx1 = -INFINITY;
-#pragma unroll
-      for (int i = 0; i < 32; i += 2) { mx0 = fmax3(mx0, t2[i].x, t2[i].y); mx1 = fmax3(mx1, t2[i + 1].x, t2[i + 1].y); }
-      float tmax = fmaxf(mx0, mx1);
-      sMx[((j & 1) * 2 + h) * 128 + r] = tmax;
-      bar_sync(3 + (warp & 3), 64);                                    // the two warps that share these 32 rows
-      tmax = fmaxf(tmax, sMx[((j & 1) * 2 + (h ^ 1)) * 128 + r]);
-      // online softmax bookkeeping (log2 domain): mt = qs * tmax is the block row max of s*log2e
-      const float mt = qs * tmax;
-      const float m_new = fmaxf(m_run, mt);
-      const float ref = P_NORM == ROTATTN_NORM_ROWBLOCK ? mt : m_new;
-      const float alpha = ex2_approx(m_run - m_new);                   // first block: exp2(-inf) = 0
-      const float beta = P_NORM == ROTATTN_NORM_ROWBLOCK ? ex2_approx(mt - m_new) : 1.f;
-      const float2 nref2 = make_float2(-ref, -ref);
-      float2 ls0 = make_float2(0.f, 0.f), ls1 = make_float2(0.f, 0.f);
-      uint32_t pw[16];
-#pragma unroll
-      for (int g = 0; g < 16; ++g) {
-        const float2 e0 = ffma2(t2[2 * g], qs2, nref2), e1 = ffma2(t2[2 * g + 1], qs2, nref2);
-        const float2 p0 = make_float2(ex2_approx(e0.x), ex2_approx(e0.y));
-        const float2 p1 = make_float2(ex2_approx(e1.x), ex2_approx(e1.y));
-        ls0 = fadd2(ls0, p0);
-        ls1 = fadd2(ls1, p1);
-        const float2 f0 = ffma2(p0, lev2, magic2), f1 = ffma2(p1, lev2, magic2);   // low byte = rne(LEVELS * p)
-        const uint32_t lo = __byte_perm(__float_as_uint(f0.x), __float_as_uint(f0.y), 0x0040);
-        const uint32_t hi = __byte_perm(__float_as_uint(f1.x), __float_as_uint(f1.y), 0x0040);
-        pw[g] = __byte_perm(lo, hi, 0x5410);
-      }
-      if (DEBUG) {
-#pragma unroll
-        for (int g = 0; g < 16; ++g) *reinterpret_cast<uint32_t*>(a.P_dump + (size_t)r * a.npad + j * kTile + cb + g * 4) = pw[g];
-      }
-      tmem_st16(tmem_base + lane_off + TM_S + b * 128 + 16 * h, pw);   // u8 P tile aliases S columns [0,32)
-      if (h == 0) sAB[(j % AB_RING) * 128 + r] = make_float2(alpha, beta * (1.f / LEVELS));
-      l_run = alpha * l_run + beta * ((ls0.x + ls0.y) + (ls1.x + ls1.y));
-      m_run = m_new;
+      sAB[(j % AB_RING) * 128 + r] = make_float2(mt, (ls0.x + ls0.y) + (ls1.x + ls1.y));
       tmem_wait_st();
       tc_fence_before();
-      mbar_arrive(&p_full[b]);
-      if (h == 0) {
-        mbar_arrive(&ab_full[j % AB_RING]);
-        if (j + 1 < nblk) sKs[(b ^ 1) * 128 + r] = ks_next;
-      }
+      mbar_arrive(&p_full[g]);
+      mbar_arrive(&ab_full[j % AB_RING]);
+      mbar_arrive(&ks_empty[ring]);
     }
-    sL[h * 128 + r] = l_run;
-    mbar_arrive(l_full);
   } else {
     // ------------------------------------------------------------------ drain: 2 threads per query row of O
     asm volatile("setmaxnreg.inc.sync.aligned.u32 120;");
     constexpr int DH = D / 2;                      // channels per thread
+    constexpr float INV_LEVELS = P_MODE == ROTATTN_P_ASYM15 ? 1.f / 15.f : 1.f / 7.f;
     const int tdr = threadIdx.x - 384;
     const int h = tdr >> 7, r = tdr & 127;
     const int row = q0 + r;
     const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
-    const float* vsrc = a.Vs + (size_t)bh * nblk * D;
     float2 o2[DH / 2];
 #pragma unroll
     for (int d = 0; d < DH / 2; ++d) o2[d] = make_float2(0.f, 0.f);
-    if (tdr < D) sVs[tdr] = vsrc[tdr];
+    float m_run = -INFINITY, l_run = 0.f;
     for (int j = 0; j < nblk; ++j) {
       const int b = j & 1;
-      bar_sync(2, 256);
-      float vs_next = 0.f;
-      if (j + 1 < nblk && tdr < D) vs_next = vsrc[(size_t)(j + 1) * D + tdr];
-      const float2* vsb2 = reinterpret_cast<const float2*>(sVs + b * D + h * DH);
+      // online softmax bookkeeping (L157): m' = max(m, mt); alpha = exp(m - m'); beta = exp(mt - m'); l = alpha l + beta sum(P^)
       mbar_wait(&ab_full[j % AB_RING], (j / AB_RING) & 1);
-      const float2 ab = sAB[(j % AB_RING) * 128 + r];
+      const float2 ms = sAB[(j % AB_RING) * 128 + r];
+      const float m_new = fmaxf(m_run, ms.x);
+      const float alpha = ex2_approx(m_run - m_new);                   // first block: exp2(-inf) = 0
+      const float beta = ex2_approx(ms.x - m_new);
+      l_run = alpha * l_run + beta * ms.y;
+      m_run = m_new;
+      const float cf = beta * INV_LEVELS;
+      const float2 c2 = make_float2(cf, cf), a2 = make_float2(alpha, alpha);
+      const bool keep = __all_sync(0xffffffffu, alpha == 1.f);         // no new row max in this warp's 32 rows
+      const int vring = j % VS_RING;
+      mbar_wait(&vs_full[vring], (j / VS_RING) & 1);
+      const float2* vsb2 = reinterpret_cast<const float2*>(sVs + vring * D + h * DH);
       mbar_wait(&pv_full[b], (j >> 1) & 1);
       tc_fence_after();
-      const float2 c2 = make_float2(ab.y, ab.y), a2 = make_float2(ab.x, ab.x);
-      const bool keep = __all_sync(0xffffffffu, ab.x == 1.f);          // no new row max in this warp's 32 rows
 #pragma unroll
       for (int cc = 0; cc < DH / 32; ++cc) {
         uint32_t v[32];
@@ -323,10 +337,9 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           }
         }
       }
-      if (j + 1 < nblk && tdr < D) sVs[(b ^ 1) * D + tdr] = vs_next;
+      mbar_arrive(&vs_empty[vring]);
     }
-    mbar_wait(l_full, 0);
-    const float inv_l = 1.f / (sL[r] + sL[128 + r]);
+    const float inv_l = 1.f / l_run;
     if (row < a.N) {
       __half* dst = (DEBUG ? a.O + (size_t)r * D : a.O + ((size_t)bh * a.N + row) * D) + h * DH;
 #pragma unroll
@@ -353,16 +366,13 @@ template <int D, bool DEBUG>
 int launch_variant(const rotattn_params& p, const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv,
                    const FwdInt4Args& a, dim3 grid, cudaStream_t cs) {
   constexpr int smem = SmemInt4<D>::TOTAL;
-#define ROTATTN_LAUNCH(PM, PN)                                                                                      \
-  do {                                                                                                              \
-    ROTATTN_CUDA_TRY(cudaFuncSetAttribute(fwd_int4_kernel<D, PM, PN, DEBUG>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); \
-    fwd_int4_kernel<D, PM, PN, DEBUG><<<grid, kInt4Threads, smem, cs>>>(tq, tk, tv, a);                                      \
-  } while (0)
-  if (p.p_mode == ROTATTN_P_ASYM15 && p.p_norm == ROTATTN_NORM_ROWBLOCK) ROTATTN_LAUNCH(ROTATTN_P_ASYM15, ROTATTN_NORM_ROWBLOCK);
-  else if (p.p_mode == ROTATTN_P_ASYM15) ROTATTN_LAUNCH(ROTATTN_P_ASYM15, ROTATTN_NORM_RUNNING);
-  else if (p.p_norm == ROTATTN_NORM_ROWBLOCK) ROTATTN_LAUNCH(ROTATTN_P_SYM7, ROTATTN_NORM_ROWBLOCK);
-  else ROTATTN_LAUNCH(ROTATTN_P_SYM7, ROTATTN_NORM_RUNNING);
-#undef ROTATTN_LAUNCH
+  if (p.p_mode == ROTATTN_P_ASYM15) {
+    ROTATTN_CUDA_TRY(cudaFuncSetAttribute(fwd_int4_kernel<D, ROTATTN_P_ASYM15, DEBUG>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    fwd_int4_kernel<D, ROTATTN_P_ASYM15, DEBUG><<<grid, kInt4Threads, smem, cs>>>(tq, tk, tv, a);
+  } else {
+    ROTATTN_CUDA_TRY(cudaFuncSetAttribute(fwd_int4_kernel<D, ROTATTN_P_SYM7, DEBUG>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    fwd_int4_kernel<D, ROTATTN_P_SYM7, DEBUG><<<grid, kInt4Threads, smem, cs>>>(tq, tk, tv, a);
+  }
   ROTATTN_CUDA_TRY(cudaGetLastError());
   return ROTATTN_OK;
 }
@@ -403,6 +413,7 @@ int fwd_int4_common(const rotattn_params* p, const uint8_t* Q4, const float* Qs,
   a.N = p->N; a.nblk = nblk; a.npad = ws.npad; a.dbg_bh = bh; a.dbg_qtile = q_tile;
   a.scale_log2 = (float)(1.4426950408889634 / std::sqrt((double)p->D));
   dim3 grid(debug ? 1 : nblk, debug ? 1 : (head_sel ? n_sel : BH));
+  if (p->p_norm == ROTATTN_NORM_RUNNING) return launch_fwd_int4_sync(*p, tq, tk, tv, a, grid, debug, cs);
   if (p->D == 128) return debug ? launch_variant<128, true>(*p, tq, tk, tv, a, grid, cs) : launch_variant<128, false>(*p, tq, tk, tv, a, grid, cs);
   return debug ? launch_variant<64, true>(*p, tq, tk, tv, a, grid, cs) : launch_variant<64, false>(*p, tq, tk, tv, a, grid, cs);
 }

@@ -1,0 +1,33 @@
+// Shared declarations of the two INT4 attention kernels (fwd_int4.cu: ROWBLOCK normaliser, block-independent
+// softmax; fwd_int4_sync.cu: RUNNING normaliser, softmax serialised over KV blocks).
+#pragma once
+#include "tc_common.cuh"
+
+namespace rotattn {
+
+constexpr int kInt4Threads = 640;
+
+struct FwdInt4Args {
+  const float* Qs;        // [BH, N]
+  const float* Ks;        // [BH, N]
+  const float* Vs;        // [BH, nG, D]
+  __half* O;              // [BH, N, D]  (debug: [128, D] tile)
+  const int32_t* head_sel;
+  int32_t* S_dump;        // debug only
+  uint8_t* P_dump;        // debug only
+  int N, nblk, npad;
+  int dbg_bh, dbg_qtile;  // debug only
+  float scale_log2;       // log2(e) / sqrt(D)
+};
+
+__device__ __forceinline__ float ex2_approx(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+// RUNNING-normaliser kernel (fwd_int4_sync.cu)
+int launch_fwd_int4_sync(const rotattn_params& p, const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv,
+                         const FwdInt4Args& a, dim3 grid, bool debug, cudaStream_t cs);
+
+}  // namespace rotattn
