@@ -50,7 +50,7 @@ template <bool MASK>
 __device__ __forceinline__ void chunk_scale(const uint32_t (&v)[32], const float2* ks2, int nvalid_rel, float2 (&t2)[16]) {
 #pragma unroll
   for (int i = 0; i < 16; ++i) {
-    t2[i] = fmul2(make_float2((float)(int32_t)v[2 * i], (float)(int32_t)v[2 * i + 1]), ks2[i]);
+    t2[i] = fmul2(make_float2(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1])), ks2[i]);
     if (MASK) {
       if (2 * i >= nvalid_rel) t2[i].x = -INFINITY;
       if (2 * i + 1 >= nvalid_rel) t2[i].y = -INFINITY;
@@ -164,8 +164,8 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     } else if (warp == 1) {
       // ---------------------------------------------------------------- MMA issuer
       if (lane == 0) {
-        constexpr uint32_t idesc_s = umma_idesc(2, 1, 1, 128, 128);      // s32 <- s8 x s8
-        constexpr uint32_t idesc_pv = umma_idesc(2, 0, 1, 128, D);       // s32 <- u8 x s8
+        constexpr uint32_t idesc_s = umma_idesc(1, 0, 0, 128, 128);      // f32 <- e4m3 x e4m3 (integer codes * 2^-9)
+        constexpr uint32_t idesc_pv = umma_idesc(1, 0, 0, 128, D);       // f32 <- e4m3 x e4m3
         constexpr int KSTEPS_S = D / 32;                                 // D=64 rows are zero-padded to 128 B
         const uint64_t qd = umma_desc_k128(smem_u32(sQ));
         auto issue_s = [&](int m) {                                      // S(m) -> buffer m & 1
@@ -175,7 +175,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           const uint64_t kd = umma_desc_k128(smem_u32(sK + st * L::K_BYTES));
 #pragma unroll
           for (int k = 0; k < KSTEPS_S; ++k)
-            mma_ss<MmaKind::I8>(tmem_base + TM_S + (m & 1) * 128, qd + 2 * k, kd + 2 * k, idesc_s, k != 0);
+            mma_ss<MmaKind::F8F6F4>(tmem_base + TM_S + (m & 1) * 128, qd + 2 * k, kd + 2 * k, idesc_s, k != 0);
           tc_commit(&k_empty[st]);
           tc_commit(&s_full[m & 1]);
         };
@@ -192,7 +192,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           const uint64_t vd = umma_desc_k128(smem_u32(sV + vst * L::V_BYTES));
 #pragma unroll
           for (int k = 0; k < 4; ++k)
-            mma_ts<MmaKind::I8>(tmem_base + TM_PV + b * 128, tmem_base + TM_S + b * 128 + 8 * k, vd + 2 * k, idesc_pv, k != 0);
+            mma_ts<MmaKind::F8F6F4>(tmem_base + TM_PV + b * 128, tmem_base + TM_S + b * 128 + 8 * k, vd + 2 * k, idesc_pv, k != 0);
           tc_commit(&v_empty[vst]);
           tc_commit(&pv_full[b]);
           if (j + 2 < nblk) issue_s(j + 2);                              // reuses S buffer b after P(j) was consumed
@@ -265,7 +265,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         if (c < 3) tmem_ld32(s_addr + (c + 1) * 32, nxt);
         if (DEBUG) {
 #pragma unroll
-          for (int i = 0; i < 32; ++i) a.S_dump[(size_t)r * a.npad + j * kTile + c * 32 + i] = (int32_t)cur[i];
+          for (int i = 0; i < 32; ++i) a.S_dump[(size_t)r * a.npad + j * kTile + c * 32 + i] = (int32_t)(__uint_as_float(cur[i]) * kAccScale);
         }
         uint32_t pw[8];
         if (ragged) chunk_exp<true, P_MODE>(cur, ks2 + c * 16, nvalid - c * 32, qs2, nref2, ls0, ls1, pw);
@@ -287,7 +287,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     // ------------------------------------------------------------------ drain: 2 threads per query row of O
     asm volatile("setmaxnreg.inc.sync.aligned.u32 120;");
     constexpr int DH = D / 2;                      // channels per thread
-    constexpr float INV_LEVELS = P_MODE == ROTATTN_P_ASYM15 ? 1.f / 15.f : 1.f / 7.f;
+    constexpr float INV_LEVELS = kAccScale * (P_MODE == ROTATTN_P_ASYM15 ? 1.f / 15.f : 1.f / 7.f);   // undoes the 2^-18 of the E4M3 code products
     const int tdr = threadIdx.x - 384;
     const int h = tdr >> 7, r = tdr & 127;
     const int row = q0 + r;
@@ -326,13 +326,13 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         if (keep) {
 #pragma unroll
           for (int d = 0; d < 16; ++d) {
-            const float2 y = fmul2(make_float2((float)(int32_t)v[2 * d], (float)(int32_t)v[2 * d + 1]), vsb2[cc * 16 + d]);
+            const float2 y = fmul2(make_float2(__uint_as_float(v[2 * d]), __uint_as_float(v[2 * d + 1])), vsb2[cc * 16 + d]);
             o2[cc * 16 + d] = ffma2(y, c2, o2[cc * 16 + d]);           // O += (beta/levels) * pv * Vs[g][d]
           }
         } else {
 #pragma unroll
           for (int d = 0; d < 16; ++d) {
-            const float2 y = fmul2(make_float2((float)(int32_t)v[2 * d], (float)(int32_t)v[2 * d + 1]), vsb2[cc * 16 + d]);
+            const float2 y = fmul2(make_float2(__uint_as_float(v[2 * d]), __uint_as_float(v[2 * d + 1])), vsb2[cc * 16 + d]);
             o2[cc * 16 + d] = ffma2(o2[cc * 16 + d], a2, fmul2(y, c2));   // O = alpha O + (beta/levels) * pv * Vs[g][d]
           }
         }
@@ -411,7 +411,7 @@ int fwd_int4_common(const rotattn_params* p, const uint8_t* Q4, const float* Qs,
   a.Qs = Qs; a.Ks = Ks; a.Vs = Vs; a.O = (__half*)O; a.head_sel = head_sel;
   a.S_dump = S_dump; a.P_dump = P_dump;
   a.N = p->N; a.nblk = nblk; a.npad = ws.npad; a.dbg_bh = bh; a.dbg_qtile = q_tile;
-  a.scale_log2 = (float)(1.4426950408889634 / std::sqrt((double)p->D));
+  a.scale_log2 = (float)(1.4426950408889634 / std::sqrt((double)p->D) * (double)kAccScale);   // S arrives as acc * 2^-18
   dim3 grid(debug ? 1 : nblk, debug ? 1 : (head_sel ? n_sel : BH));
   if (p->p_norm == ROTATTN_NORM_RUNNING) return launch_fwd_int4_sync(*p, tq, tk, tv, a, grid, debug, cs);
   if (p->D == 128) return debug ? launch_variant<128, true>(*p, tq, tk, tv, a, grid, cs) : launch_variant<128, false>(*p, tq, tk, tv, a, grid, cs);

@@ -6,6 +6,9 @@
 namespace rotattn {
 
 constexpr int kInt4Threads = 640;
+// The widened operands are E4M3 bytes that encode code * 2^-9 (see prologue.cu: code_byte), so both tensor products
+// arrive in tensor memory as fp32 values  integer_accumulator * 2^-18  (exact: |acc| <= 13440 < 2^24).
+constexpr float kAccScale = 262144.f;
 
 struct FwdInt4Args {
   const float* Qs;        // [BH, N]
@@ -17,7 +20,7 @@ struct FwdInt4Args {
   uint8_t* P_dump;        // debug only
   int N, nblk, npad;
   int dbg_bh, dbg_qtile;  // debug only
-  float scale_log2;       // log2(e) / sqrt(D)
+  float scale_log2;       // 2^18 * log2(e) / sqrt(D)
 };
 
 __device__ __forceinline__ float ex2_approx(float x) {

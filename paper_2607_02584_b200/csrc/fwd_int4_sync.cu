@@ -103,8 +103,8 @@ fwd_int4_sync_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
     } else if (warp == 1) {
       // ---------------------------------------------------------------- MMA issuer
       if (lane == 0) {
-        constexpr uint32_t idesc_s = umma_idesc(2, 1, 1, 128, 128);      // s32 <- s8 x s8
-        constexpr uint32_t idesc_pv = umma_idesc(2, 0, 1, 128, D);       // s32 <- u8 x s8
+        constexpr uint32_t idesc_s = umma_idesc(1, 0, 0, 128, 128);      // f32 <- e4m3 x e4m3 (integer codes * 2^-9)
+        constexpr uint32_t idesc_pv = umma_idesc(1, 0, 0, 128, D);       // f32 <- e4m3 x e4m3
         constexpr int KSTEPS_S = D / 32;                                 // D=64 rows are zero-padded to 128 B
         const uint64_t qd = umma_desc_k128(smem_u32(sQ));
         mbar_wait(q_full, 0);
@@ -113,7 +113,7 @@ fwd_int4_sync_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
         {
           const uint64_t kd = umma_desc_k128(smem_u32(sK));
 #pragma unroll
-          for (int k = 0; k < KSTEPS_S; ++k) mma_ss<MmaKind::I8>(tmem_base + TM_S, qd + 2 * k, kd + 2 * k, idesc_s, k != 0);
+          for (int k = 0; k < KSTEPS_S; ++k) mma_ss<MmaKind::F8F6F4>(tmem_base + TM_S, qd + 2 * k, kd + 2 * k, idesc_s, k != 0);
           tc_commit(&k_empty[0]);
           tc_commit(&s_full[0]);
         }
@@ -128,7 +128,7 @@ fwd_int4_sync_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
             const uint64_t kd = umma_desc_k128(smem_u32(sK + ks * L::K_BYTES));
 #pragma unroll
             for (int k = 0; k < KSTEPS_S; ++k)
-              mma_ss<MmaKind::I8>(tmem_base + TM_S + (b ^ 1) * 128, qd + 2 * k, kd + 2 * k, idesc_s, k != 0);
+              mma_ss<MmaKind::F8F6F4>(tmem_base + TM_S + (b ^ 1) * 128, qd + 2 * k, kd + 2 * k, idesc_s, k != 0);
             tc_commit(&k_empty[ks]);
             tc_commit(&s_full[b ^ 1]);
             ++ks;
@@ -140,7 +140,7 @@ fwd_int4_sync_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
           const uint64_t vd = umma_desc_k128(smem_u32(sV + vs * L::V_BYTES));
 #pragma unroll
           for (int k = 0; k < 4; ++k)
-            mma_ts<MmaKind::I8>(tmem_base + TM_PV + b * 128, tmem_base + TM_S + b * 128 + 8 * k, vd + 2 * k, idesc_pv, k != 0);
+            mma_ts<MmaKind::F8F6F4>(tmem_base + TM_PV + b * 128, tmem_base + TM_S + b * 128 + 8 * k, vd + 2 * k, idesc_pv, k != 0);
           tc_commit(&v_empty[vs]);
           tc_commit(&pv_full[b]);
           if (++vs == KS_STAGES) { vs = 0; vph ^= 1; }
@@ -181,14 +181,14 @@ fwd_int4_sync_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
         if (DEBUG) {
 #pragma unroll
           for (int i = 0; i < 32; ++i) {
-            a.S_dump[(size_t)r * a.npad + j * kTile + cb + i] = (int32_t)v0[i];
-            a.S_dump[(size_t)r * a.npad + j * kTile + cb + 32 + i] = (int32_t)v1[i];
+            a.S_dump[(size_t)r * a.npad + j * kTile + cb + i] = (int32_t)(__uint_as_float(v0[i]) * kAccScale);
+            a.S_dump[(size_t)r * a.npad + j * kTile + cb + 32 + i] = (int32_t)(__uint_as_float(v1[i]) * kAccScale);
           }
         }
 #pragma unroll
         for (int i = 0; i < 16; ++i) {                                 // t = acc * Ks_j * log2e/sqrt(D)
-          t2[i] = fmul2(make_float2((float)(int32_t)v0[2 * i], (float)(int32_t)v0[2 * i + 1]), ksb2[i]);
-          t2[16 + i] = fmul2(make_float2((float)(int32_t)v1[2 * i], (float)(int32_t)v1[2 * i + 1]), ksb2[16 + i]);
+          t2[i] = fmul2(make_float2(__uint_as_float(v0[2 * i]), __uint_as_float(v0[2 * i + 1])), ksb2[i]);
+          t2[16 + i] = fmul2(make_float2(__uint_as_float(v1[2 * i]), __uint_as_float(v1[2 * i + 1])), ksb2[16 + i]);
         }
       }
       if (nvalid < kTile) {                                            // keys >= N: masked out of max, sum and codes
@@ -231,7 +231,7 @@ fwd_int4_sync_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
         for (int g = 0; g < 16; ++g) *reinterpret_cast<uint32_t*>(a.P_dump + (size_t)r * a.npad + j * kTile + cb + g * 4) = pw[g];
       }
       tmem_st16(tmem_base + lane_off + TM_S + b * 128 + 16 * h, pw);   // u8 P tile aliases S columns [0,32)
-      if (h == 0) sAB[(j % KS_RING) * 128 + r] = make_float2(alpha, beta * (1.f / LEVELS));
+      if (h == 0) sAB[(j % KS_RING) * 128 + r] = make_float2(alpha, beta * (kAccScale / LEVELS));
       l_run = alpha * l_run + beta * ((ls0.x + ls0.y) + (ls1.x + ls1.y));
       m_run = m_new;
       tmem_wait_st();
@@ -281,13 +281,13 @@ fwd_int4_sync_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
         if (keep) {
 #pragma unroll
           for (int d = 0; d < 16; ++d) {
-            const float2 y = fmul2(make_float2((float)(int32_t)v[2 * d], (float)(int32_t)v[2 * d + 1]), vsb2[cc * 16 + d]);
+            const float2 y = fmul2(make_float2(__uint_as_float(v[2 * d]), __uint_as_float(v[2 * d + 1])), vsb2[cc * 16 + d]);
             o2[cc * 16 + d] = ffma2(y, c2, o2[cc * 16 + d]);           // O += (beta/levels) * pv * Vs[g][d]
           }
         } else {
 #pragma unroll
           for (int d = 0; d < 16; ++d) {
-            const float2 y = fmul2(make_float2((float)(int32_t)v[2 * d], (float)(int32_t)v[2 * d + 1]), vsb2[cc * 16 + d]);
+            const float2 y = fmul2(make_float2(__uint_as_float(v[2 * d]), __uint_as_float(v[2 * d + 1])), vsb2[cc * 16 + d]);
             o2[cc * 16 + d] = ffma2(o2[cc * 16 + d], a2, fmul2(y, c2));   // O = alpha O + (beta/levels) * pv * Vs[g][d]
           }
         }

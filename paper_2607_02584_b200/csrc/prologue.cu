@@ -24,6 +24,10 @@ __device__ __forceinline__ int quant_code(float y, float inv) {
   int c = __float2int_rn(__fmul_rn(y, inv));       // round half to even
   return max(-7, min(7, c));
 }
+// Widened MMA operand byte of a code c in [-7,7] (or a P code in [0,15]): sign-magnitude, which is the E4M3
+// encoding of c * 2^-9 (E4M3 subnormals are m * 2^-9, and bytes 8..15 are the first normal binade 2^-6 * (1 + m/8)),
+// so tcgen05 kind::f8f6f4 multiplies and accumulates the integer codes exactly, scaled by 2^-18, in fp32.
+__device__ __forceinline__ uint32_t code_byte(int c) { return (uint32_t)(abs(c) | ((c >> 24) & 0x80)); }
 
 template <int D, int ROT>
 __global__ void __launch_bounds__(256) prepare_qk_kernel(const PrepArgs a) {
@@ -132,10 +136,10 @@ __global__ void __launch_bounds__(256) prepare_qk_kernel(const PrepArgs a) {
       if (a.X8[m]) {
         int8_t* dst = a.X8[m] + tok * kQKRowBytes;
         if (CPL == 4) {
-          uint32_t w = (uint32_t)(c[0] & 0xFF) | ((uint32_t)(c[1] & 0xFF) << 8) | ((uint32_t)(c[2] & 0xFF) << 16) | ((uint32_t)(c[3] & 0xFF) << 24);
+          uint32_t w = code_byte(c[0]) | (code_byte(c[1]) << 8) | (code_byte(c[2]) << 16) | (code_byte(c[3]) << 24);
           *reinterpret_cast<uint32_t*>(dst + lane * 4) = w;
         } else {
-          *reinterpret_cast<uint16_t*>(dst + lane * 2) = (uint16_t)((c[0] & 0xFF) | ((c[1] & 0xFF) << 8));
+          *reinterpret_cast<uint16_t*>(dst + lane * 2) = (uint16_t)(code_byte(c[0]) | (code_byte(c[1]) << 8));
           *reinterpret_cast<uint16_t*>(dst + 64 + lane * 2) = 0;      // zero pad to a 128-byte row
         }
       }
@@ -223,7 +227,7 @@ __global__ void __launch_bounds__(256) quant_v_kernel(const __half* __restrict__
       for (int j = 0; j < 8; ++j) {
         int c = quant_code(__half2float(h[j]), inv[j]);
         pk |= (uint32_t)(c & 0xF) << (4 * j);
-        tw[j] |= (uint32_t)(c & 0xFF) << (8 * r);
+        tw[j] |= code_byte(c) << (8 * r);
       }
       int row = (q0 + ps * QPP) * 4 + r;
       if (row0 + row < N) *reinterpret_cast<uint32_t*>(V4 + (bh * N + row0 + row) * (long long)(D / 2) + cc * 4) = pk;
@@ -259,7 +263,7 @@ __global__ void unpack_qk_kernel(const uint8_t* __restrict__ X4, int8_t* __restr
   if (w * 4 < D) {
     const uint16_t pk = *reinterpret_cast<const uint16_t*>(X4 + tok * (D / 2) + w * 2);
 #pragma unroll
-    for (int j = 0; j < 4; ++j) out |= (uint32_t)(nib2int((pk >> (4 * j)) & 0xF) & 0xFF) << (8 * j);
+    for (int j = 0; j < 4; ++j) out |= code_byte(nib2int((pk >> (4 * j)) & 0xF)) << (8 * j);
   }
   *reinterpret_cast<uint32_t*>(X8 + tok * kQKRowBytes + w * 4) = out;
 }
@@ -272,8 +276,8 @@ __global__ void unpack_vt_kernel(const uint8_t* __restrict__ V4, int8_t* __restr
   for (int i = threadIdx.x; i < kTile * (D / 2); i += blockDim.x) {
     int r = i / (D / 2), b = i % (D / 2);
     uint8_t pk = (row0 + r < N) ? V4[(bh * N + row0 + r) * (long long)(D / 2) + b] : 0;
-    tile[2 * b][r] = (int8_t)nib2int(pk & 0xF);
-    tile[2 * b + 1][r] = (int8_t)nib2int(pk >> 4);
+    tile[2 * b][r] = (int8_t)code_byte(nib2int(pk & 0xF));
+    tile[2 * b + 1][r] = (int8_t)code_byte(nib2int(pk >> 4));
   }
   __syncthreads();
   for (int i = threadIdx.x; i < D * kTile; i += blockDim.x) {

@@ -57,9 +57,14 @@ def _check_head(po, tab, b, q, k, v, bi, h, rot=None, check_ws=True):
         npad = -(-N // 128) * 128
         qk_bytes = -(-BH * N * 128 // 1024) * 1024
         ws = b.ws.cpu().numpy()
-        q8 = ws[:BH * N * 128].view(np.int8).reshape(BH, N, 128)[bh]
-        k8 = ws[qk_bytes:qk_bytes + BH * N * 128].view(np.int8).reshape(BH, N, 128)[bh]
-        v8t = ws[2 * qk_bytes:2 * qk_bytes + BH * D * npad].view(np.int8).reshape(BH, D, npad)[bh]
+
+        def codes(x):      # widened operand bytes are sign-magnitude (= E4M3 encoding of code * 2^-9)
+            x = x.view(np.uint8).astype(np.int32)
+            assert not np.any(x == 0x80), 'negative zero byte'
+            return np.where(x & 0x80, -(x & 0x7F), x & 0x7F).astype(np.int8)
+        q8 = codes(ws[:BH * N * 128]).reshape(BH, N, 128)[bh]
+        k8 = codes(ws[qk_bytes:qk_bytes + BH * N * 128]).reshape(BH, N, 128)[bh]
+        v8t = codes(ws[2 * qk_bytes:2 * qk_bytes + BH * D * npad]).reshape(BH, D, npad)[bh]
         assert np.array_equal(q8[:, :D], pq['q_codes']) and np.all(q8[:, D:] == 0)
         assert np.array_equal(k8[:, :D], pq['k_codes'])
         assert np.array_equal(v8t[:, :N], vc.T) and np.all(v8t[:, N:] == 0)
