@@ -1,29 +1,34 @@
-// rotattn_fwd_int4 (steps a4-a9): INT4 FlashAttention forward on tcgen05 kind::i8, row-block P normaliser.
+// rotattn_fwd_int4 (steps a4-a9): INT4 FlashAttention forward on tcgen05 (kind::f8f6f4 on integer-exact E4M3 code
+// bytes, see fwd_int4.cuh), row-block P normaliser.
 //
-// One CTA = one 128-row query tile of one (b,h); 20 warps, warp-specialised:
-//   warp 0        TMA producer : Q tile once, K / V^T tiles through 3-stage shared-memory rings
-//   warp 1        MMA issuer   : S = Q K^T (int8 x int8 -> int32, TMEM), P~V (u8 from TMEM x int8 -> int32, TMEM)
+// One CTA = one 128-row query tile of one (b,h); 28 warps, warp-specialised:
+//   warp 0        TMA producer : Q tile once, K tiles (4-stage ring) and V^T tiles (3-stage ring)
+//   warp 1        MMA issuer   : S = Q K^T (codes x codes, exact, TMEM), P~V (P codes from TMEM x V codes, TMEM)
 //   warp 2        TMEM allocator, then V-scale loader (Vs[g][:] -> shared ring)
-//   warp 3        K-scale loader (Ks[j] * log2e/sqrt(D) -> shared ring)
-//   warps 4-7     softmax group A: even KV blocks, one thread per query row
-//   warps 8-11    softmax group B: odd KV blocks
-//   warps 12-19   drain: 2 threads per query row (D/2 channels each): online-softmax bookkeeping (m, l, alpha, beta),
-//                 int32 P~V block -> fp32 O registers, epilogue O/l
+//   warp 3        K-scale loader (Ks[j] * 2^18 log2e/sqrt(D) -> shared ring)
+//   warps 4-11    softmax group 0: even KV blocks; warps 4-7 own keys [0,64) of the block, warps 8-11 keys [64,128)
+//   warps 12-19   softmax group 1: odd KV blocks, same split  (two threads per query row and block)
+//   warps 20-27   drain: 2 threads per query row (D/2 channels each): online-softmax bookkeeping (m, l, alpha, beta),
+//                 P~V block -> fp32 O registers, epilogue O/l
 // With the row-block normaliser (reading 13) the codes of block j depend only on block j, so the two softmax
-// groups work on different blocks out of phase (one in its ALU phase while the other keeps the MUFU pipe busy) and
-// the running max lives in the drain threads.  Each softmax thread makes two passes over its S row in tensor memory
-// (pass 1: block row max, pass 2: exp2 / codes) in 32-column chunks, so it needs no 128-register row buffer.
-// TMEM (512 columns): S[2] at 0/128 (u8 P tile aliases the first 32 columns of its S buffer), PV[2] at 256/384.
+// groups work on different blocks concurrently and the running max lives in the drain threads.  Each softmax thread
+// makes two passes over its half row of S in tensor memory (pass 1: block row max, exchanged with the partner thread
+// through shared memory; pass 2: exp2 / row sum / codes) in 16-column chunks.
+// TMEM (512 columns): S[2] at 0/128, PV at 256, four P-code slots of 32 columns at 384.  P has its own slots so that
+// an S buffer is released as soon as pass 2 has read it (S(j+2) is issued before P~V(j), hiding the MMA latency).
 // The per-block drain is forced by the method: beta (row, block) and Vs (channel, block) change every KV block
-// (PAPER.md:L157 online softmax, L190 per-group V scales), so integer P~V cannot accumulate across blocks.
+// (PAPER.md:L157 online softmax, L190 per-group V scales), so P~V cannot accumulate across blocks in tensor memory.
 #include <cmath>
 #include <cstdio>
 #include "fwd_int4.cuh"
 
 namespace rotattn {
 
-constexpr int KV_STAGES = 3;
-constexpr int AB_RING = 4;
+constexpr int kFwdThreads = 896;
+constexpr int K_STAGES = 4;
+constexpr int V_STAGES = 3;
+constexpr int P_SLOTS = 4;
+constexpr int AB_RING = 8;
 constexpr int KS_RING = 4;
 constexpr int VS_RING = 4;
 
@@ -34,22 +39,23 @@ struct SmemInt4 {
   static constexpr int V_BYTES = D * 128;
   static constexpr int OFF_Q = 0;
   static constexpr int OFF_K = OFF_Q + Q_BYTES;
-  static constexpr int OFF_V = OFF_K + KV_STAGES * K_BYTES;
-  static constexpr int OFF_KS = OFF_V + KV_STAGES * V_BYTES;          // float [KS_RING][128]
+  static constexpr int OFF_V = OFF_K + K_STAGES * K_BYTES;
+  static constexpr int OFF_KS = OFF_V + V_STAGES * V_BYTES;           // float [KS_RING][128]
   static constexpr int OFF_VS = OFF_KS + KS_RING * 128 * 4;           // float [VS_RING][D]
-  static constexpr int OFF_AB = OFF_VS + VS_RING * D * 4;             // float2 [AB_RING][128]  (block max, block sum)
-  static constexpr int OFF_BAR = OFF_AB + AB_RING * 128 * 8;          // mbarriers
-  static constexpr int NBAR = 1 + 4 * KV_STAGES + 2 + 2 + 2 + 2 + AB_RING + 2 * KS_RING + 2 * VS_RING;
+  static constexpr int OFF_AB = OFF_VS + VS_RING * D * 4;             // float2 [AB_RING][2 halves][128]  (block max, half-row sum)
+  static constexpr int OFF_MX = OFF_AB + AB_RING * 2 * 128 * 8;       // float [2 groups][2 parities][2 halves][128]
+  static constexpr int OFF_BAR = OFF_MX + 2 * 2 * 2 * 128 * 4;        // mbarriers
+  static constexpr int NBAR = 1 + 2 * K_STAGES + 2 * V_STAGES + 2 + 2 + 2 * P_SLOTS + 2 + AB_RING + 2 * KS_RING + 2 * VS_RING;
   static constexpr int OFF_TMEM = OFF_BAR + NBAR * 8;
   static constexpr int TOTAL = OFF_TMEM + 16;
 };
 
-// ---- per-chunk element-wise work of the softmax threads (32 S columns of one query row) -------------------------
-// t = acc * Ks_j * log2e/sqrt(D) (the query scale Qs_i > 0 is applied after the max); keys >= N are masked to -inf.
+// ---- per-chunk element-wise work of the softmax threads (16 S columns of one query row) -------------------------
+// t = S * (Ks_j * 2^18 log2e/sqrt(D)) (the query scale Qs_i > 0 is applied after the max); keys >= N are masked to -inf.
 template <bool MASK>
-__device__ __forceinline__ void chunk_scale(const uint32_t (&v)[32], const float2* ks2, int nvalid_rel, float2 (&t2)[16]) {
+__device__ __forceinline__ void chunk_scale(const uint32_t (&v)[16], const float2* ks2, int nvalid_rel, float2 (&t2)[8]) {
 #pragma unroll
-  for (int i = 0; i < 16; ++i) {
+  for (int i = 0; i < 8; ++i) {
     t2[i] = fmul2(make_float2(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1])), ks2[i]);
     if (MASK) {
       if (2 * i >= nvalid_rel) t2[i].x = -INFINITY;
@@ -59,30 +65,29 @@ __device__ __forceinline__ void chunk_scale(const uint32_t (&v)[32], const float
 }
 
 template <bool MASK>
-__device__ __forceinline__ void chunk_max(const uint32_t (&v)[32], const float2* ks2, int nvalid_rel, float& mx0, float& mx1) {
-  float2 t2[16];
+__device__ __forceinline__ void chunk_max(const uint32_t (&v)[16], const float2* ks2, int nvalid_rel, float& mx0, float& mx1) {
+  float2 t2[8];
   chunk_scale<MASK>(v, ks2, nvalid_rel, t2);
 #pragma unroll
-  for (int i = 0; i < 16; i += 2) { mx0 = fmax3(mx0, t2[i].x, t2[i].y); mx1 = fmax3(mx1, t2[i + 1].x, t2[i + 1].y); }
+  for (int i = 0; i < 8; i += 2) { mx0 = fmax3(mx0, t2[i].x, t2[i].y); mx1 = fmax3(mx1, t2[i + 1].x, t2[i + 1].y); }
 }
 
-// P^ = exp2(t * Qs_i - mt); codes u = rne(LEVELS * P^) taken from the low byte of fma(P^, LEVELS, 1.5 * 2^23)
-// (Eq.12 L166-168 with the fixed scale 15 / Eq.11 L161 with 7); four codes per 32-bit TMEM column.
-template <bool MASK, int P_MODE>
-__device__ __forceinline__ void chunk_exp(const uint32_t (&v)[32], const float2* ks2, int nvalid_rel, float2 qs2, float2 nref2,
-                                          float2& ls0, float2& ls1, uint32_t (&pw)[8]) {
-  constexpr float LEVELS = P_MODE == ROTATTN_P_ASYM15 ? 15.f : 7.f;
-  const float2 lev2 = make_float2(LEVELS, LEVELS), magic2 = make_float2(12582912.f, 12582912.f);
-  float2 t2[16];
+// LEVELS * P^ = exp2(t * Qs_i - mt + log2(LEVELS)); codes u = rne(LEVELS * P^) taken from the low byte of
+// (LEVELS * P^) + 1.5 * 2^23 (Eq.12 L166-168 with the fixed scale 15 / Eq.11 L161 with 7); four codes per TMEM column.
+template <bool MASK>
+__device__ __forceinline__ void chunk_exp(const uint32_t (&v)[16], const float2* ks2, int nvalid_rel, float2 qs2, float2 nref2,
+                                          float2& ls0, float2& ls1, uint32_t (&pw)[4]) {
+  const float2 magic2 = make_float2(12582912.f, 12582912.f);
+  float2 t2[8];
   chunk_scale<MASK>(v, ks2, nvalid_rel, t2);
 #pragma unroll
-  for (int g = 0; g < 8; ++g) {
+  for (int g = 0; g < 4; ++g) {
     const float2 e0 = ffma2(t2[2 * g], qs2, nref2), e1 = ffma2(t2[2 * g + 1], qs2, nref2);
     const float2 p0 = make_float2(ex2_approx(e0.x), ex2_approx(e0.y));
     const float2 p1 = make_float2(ex2_approx(e1.x), ex2_approx(e1.y));
     ls0 = fadd2(ls0, p0);
     ls1 = fadd2(ls1, p1);
-    const float2 f0 = ffma2(p0, lev2, magic2), f1 = ffma2(p1, lev2, magic2);
+    const float2 f0 = fadd2(p0, magic2), f1 = fadd2(p1, magic2);
     const uint32_t lo = __byte_perm(__float_as_uint(f0.x), __float_as_uint(f0.y), 0x0040);
     const uint32_t hi = __byte_perm(__float_as_uint(f1.x), __float_as_uint(f1.y), 0x0040);
     pw[g] = __byte_perm(lo, hi, 0x5410);
@@ -90,7 +95,7 @@ __device__ __forceinline__ void chunk_exp(const uint32_t (&v)[32], const float2*
 }
 
 template <int D, int P_MODE, bool DEBUG>
-__global__ void __launch_bounds__(kInt4Threads, 1)
+__global__ void __launch_bounds__(kFwdThreads, 1)
 fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                 const __grid_constant__ CUtensorMap tmV, const FwdInt4Args a) {
   using L = SmemInt4<D>;
@@ -101,19 +106,22 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   float* sKs = (float*)(smem + L::OFF_KS);
   float* sVs = (float*)(smem + L::OFF_VS);
   float2* sAB = (float2*)(smem + L::OFF_AB);
+  float* sMx = (float*)(smem + L::OFF_MX);
   uint64_t* bars = (uint64_t*)(smem + L::OFF_BAR);
   uint64_t* q_full = bars;
   uint64_t* k_full = q_full + 1;
-  uint64_t* k_empty = k_full + KV_STAGES;
-  uint64_t* v_full = k_empty + KV_STAGES;
-  uint64_t* v_empty = v_full + KV_STAGES;
-  uint64_t* s_full = v_empty + KV_STAGES;     // [2] MMA -> softmax group (buffer b belongs to group b)
-  uint64_t* p_full = s_full + 2;              // [2] softmax group -> MMA (count 128)
-  uint64_t* pv_full = p_full + 2;             // [2] MMA -> drain
-  uint64_t* pv_empty = pv_full + 2;           // [2] drain -> MMA (count 256)
-  uint64_t* ab_full = pv_empty + 2;           // [AB_RING] softmax -> drain (count 128)
+  uint64_t* k_empty = k_full + K_STAGES;
+  uint64_t* v_full = k_empty + K_STAGES;
+  uint64_t* v_empty = v_full + V_STAGES;
+  uint64_t* s_full = v_empty + V_STAGES;      // [2] MMA -> softmax group (buffer b belongs to group b)
+  uint64_t* s_empty = s_full + 2;             // [2] softmax group -> MMA (count 256): S buffer has been read
+  uint64_t* p_full = s_empty + 2;             // [P_SLOTS] softmax group -> MMA (count 256)
+  uint64_t* p_empty = p_full + P_SLOTS;       // [P_SLOTS] MMA -> softmax: P~V has consumed the slot
+  uint64_t* pv_full = p_empty + P_SLOTS;      // MMA -> drain
+  uint64_t* pv_empty = pv_full + 1;           // drain -> MMA (count 256)
+  uint64_t* ab_full = pv_empty + 1;           // [AB_RING] softmax -> drain (count 256)
   uint64_t* ks_full = ab_full + AB_RING;      // [KS_RING] loader -> softmax (count 32)
-  uint64_t* ks_empty = ks_full + KS_RING;     // [KS_RING] softmax -> loader (count 128)
+  uint64_t* ks_empty = ks_full + KS_RING;     // [KS_RING] softmax -> loader (count 256)
   uint64_t* vs_full = ks_empty + KS_RING;     // [VS_RING] loader -> drain (count 32)
   uint64_t* vs_empty = vs_full + VS_RING;     // [VS_RING] drain -> loader (count 256)
   uint32_t* tmem_slot = (uint32_t*)(smem + L::OFF_TMEM);
@@ -127,10 +135,13 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   if (threadIdx.x == 0) {
     if (smem_u32(smem) & 1023u) __trap();     // SWIZZLE_128B operand tiles need 1024-byte alignment
     mbar_init(q_full, 1);
-    for (int i = 0; i < KV_STAGES; ++i) { mbar_init(&k_full[i], 1); mbar_init(&k_empty[i], 1); mbar_init(&v_full[i], 1); mbar_init(&v_empty[i], 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(&s_full[i], 1); mbar_init(&p_full[i], 128); mbar_init(&pv_full[i], 1); mbar_init(&pv_empty[i], 256); }
-    for (int i = 0; i < AB_RING; ++i) mbar_init(&ab_full[i], 128);
-    for (int i = 0; i < KS_RING; ++i) { mbar_init(&ks_full[i], 32); mbar_init(&ks_empty[i], 128); }
+    for (int i = 0; i < K_STAGES; ++i) { mbar_init(&k_full[i], 1); mbar_init(&k_empty[i], 1); }
+    for (int i = 0; i < V_STAGES; ++i) { mbar_init(&v_full[i], 1); mbar_init(&v_empty[i], 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&s_full[i], 1); mbar_init(&s_empty[i], 256); }
+    for (int i = 0; i < P_SLOTS; ++i) { mbar_init(&p_full[i], 256); mbar_init(&p_empty[i], 1); }
+    mbar_init(pv_full, 1); mbar_init(pv_empty, 256);
+    for (int i = 0; i < AB_RING; ++i) mbar_init(&ab_full[i], 256);
+    for (int i = 0; i < KS_RING; ++i) { mbar_init(&ks_full[i], 32); mbar_init(&ks_empty[i], 256); }
     for (int i = 0; i < VS_RING; ++i) { mbar_init(&vs_full[i], 32); mbar_init(&vs_empty[i], 256); }
     fence_mbar_init();
   }
@@ -139,63 +150,69 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
-  constexpr uint32_t TM_S = 0, TM_PV = 256;
+  constexpr uint32_t TM_S = 0, TM_PV = 256, TM_P = 384;
 
-  // register pool of the CTA = 640 x 96; after redistribution 128 x 32 + 256 x 96 + 256 x 120 = 59392 (must not exceed it)
+  // register pool of the CTA = 896 x 72; after redistribution 128 x 24 + 512 x 72 + 256 x 96 = 64512 (exactly the pool)
   if (warp < 4) {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
     if (warp == 0) {
       // ---------------------------------------------------------------- TMA producer
       if (lane == 0) {
         tma_prefetch_desc(&tmQ); tma_prefetch_desc(&tmK); tma_prefetch_desc(&tmV);
         mbar_arrive_expect_tx(q_full, L::Q_BYTES);
         tma_load_3d(sQ, &tmQ, q_full, 0, q0, bh);
-        int s = 0; uint32_t ph = 0;
-        for (int j = 0; j < nblk; ++j) {
-          mbar_wait(&k_empty[s], ph ^ 1);
+        auto load_k = [&](int m) {
+          const int s = m % K_STAGES;
+          mbar_wait(&k_empty[s], ((m / K_STAGES) & 1) ^ 1);
           mbar_arrive_expect_tx(&k_full[s], L::K_BYTES);
-          tma_load_3d(sK + s * L::K_BYTES, &tmK, &k_full[s], 0, j * kTile, bh);
-          mbar_wait(&v_empty[s], ph ^ 1);
+          tma_load_3d(sK + s * L::K_BYTES, &tmK, &k_full[s], 0, m * kTile, bh);
+        };
+        load_k(0);
+        if (nblk > 1) load_k(1);
+        for (int j = 0; j < nblk; ++j) {
+          if (j + 2 < nblk) load_k(j + 2);
+          const int s = j % V_STAGES;
+          mbar_wait(&v_empty[s], ((j / V_STAGES) & 1) ^ 1);
           mbar_arrive_expect_tx(&v_full[s], L::V_BYTES);
           tma_load_3d(sV + s * L::V_BYTES, &tmV, &v_full[s], j * kTile, 0, bh);
-          if (++s == KV_STAGES) { s = 0; ph ^= 1; }
         }
       }
     } else if (warp == 1) {
       // ---------------------------------------------------------------- MMA issuer
       if (lane == 0) {
         constexpr uint32_t idesc_s = umma_idesc(1, 0, 0, 128, 128);      // f32 <- e4m3 x e4m3 (integer codes * 2^-9)
-        constexpr uint32_t idesc_pv = umma_idesc(1, 0, 0, 128, D);       // f32 <- e4m3 x e4m3
+        constexpr uint32_t idesc_pv = umma_idesc(1, 0, 0, 128, D);
         constexpr int KSTEPS_S = D / 32;                                 // D=64 rows are zero-padded to 128 B
         const uint64_t qd = umma_desc_k128(smem_u32(sQ));
         auto issue_s = [&](int m) {                                      // S(m) -> buffer m & 1
-          const int st = m % KV_STAGES;
-          mbar_wait(&k_full[st], (m / KV_STAGES) & 1);
+          const int st = m % K_STAGES, b = m & 1;
+          mbar_wait(&k_full[st], (m / K_STAGES) & 1);
+          if (m >= 2) mbar_wait(&s_empty[b], ((m >> 1) - 1) & 1);        // softmax has read S(m-2) out of this buffer
           tc_fence_after();
           const uint64_t kd = umma_desc_k128(smem_u32(sK + st * L::K_BYTES));
 #pragma unroll
           for (int k = 0; k < KSTEPS_S; ++k)
-            mma_ss<MmaKind::F8F6F4>(tmem_base + TM_S + (m & 1) * 128, qd + 2 * k, kd + 2 * k, idesc_s, k != 0);
+            mma_ss<MmaKind::F8F6F4>(tmem_base + TM_S + b * 128, qd + 2 * k, kd + 2 * k, idesc_s, k != 0);
           tc_commit(&k_empty[st]);
-          tc_commit(&s_full[m & 1]);
+          tc_commit(&s_full[b]);
         };
         mbar_wait(q_full, 0);
         issue_s(0);
         if (nblk > 1) issue_s(1);
         for (int j = 0; j < nblk; ++j) {
-          const int b = j & 1;
-          const int vst = j % KV_STAGES;
-          mbar_wait(&p_full[b], (j >> 1) & 1);
-          mbar_wait(&v_full[vst], (j / KV_STAGES) & 1);
-          mbar_wait(&pv_empty[b], ((j >> 1) & 1) ^ 1);
+          if (j + 2 < nblk) issue_s(j + 2);                              // goes ahead of P~V(j): only needs S(j) to be read
+          const int slot = j % P_SLOTS, vst = j % V_STAGES;
+          mbar_wait(&p_full[slot], (j / P_SLOTS) & 1);
+          mbar_wait(&v_full[vst], (j / V_STAGES) & 1);
+          mbar_wait(pv_empty, (j & 1) ^ 1);
           tc_fence_after();
           const uint64_t vd = umma_desc_k128(smem_u32(sV + vst * L::V_BYTES));
 #pragma unroll
           for (int k = 0; k < 4; ++k)
-            mma_ts<MmaKind::F8F6F4>(tmem_base + TM_PV + b * 128, tmem_base + TM_S + b * 128 + 8 * k, vd + 2 * k, idesc_pv, k != 0);
+            mma_ts<MmaKind::F8F6F4>(tmem_base + TM_PV, tmem_base + TM_P + slot * 32 + 8 * k, vd + 2 * k, idesc_pv, k != 0);
           tc_commit(&v_empty[vst]);
-          tc_commit(&pv_full[b]);
-          if (j + 2 < nblk) issue_s(j + 2);                              // reuses S buffer b after P(j) was consumed
+          tc_commit(&p_empty[slot]);
+          tc_commit(pv_full);
         }
       }
     } else if (warp == 2) {
@@ -209,7 +226,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         mbar_arrive(&vs_full[s]);
       }
     } else {
-      // ---------------------------------------------------------------- K-scale loader: Ks_j * log2e/sqrt(D)
+      // ---------------------------------------------------------------- K-scale loader: Ks_j * 2^18 log2e/sqrt(D)
       const float* ksrc = a.Ks + (size_t)bh * a.N;
       for (int j = 0; j < nblk; ++j) {
         const int s = j % KS_RING;
@@ -222,73 +239,88 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         mbar_arrive(&ks_full[s]);
       }
     }
-  } else if (warp < 12) {
-    // ------------------------------------------------------------------ softmax groups: A = even blocks, B = odd blocks
-    const int g = (warp - 4) >> 2;                   // group index = S buffer index
-    const int r = (threadIdx.x - 128) & 127;
+  } else if (warp < 20) {
+    // ------------------------------------------------------------------ softmax groups: 0 = even blocks, 1 = odd blocks
+    constexpr float LOG2_LEVELS = P_MODE == ROTATTN_P_ASYM15 ? 3.9068905956085187f : 2.8073549220576042f;
+    const int tsm = threadIdx.x - 128;
+    const int g = tsm >> 8;                          // group index = S buffer index
+    const int h = (tsm >> 7) & 1;                    // which 64 keys of the block
+    const int r = tsm & 127;
     const int row = q0 + r;
+    const int cb = 64 * h;
     const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
     // qs >= 1e-30 keeps (-inf) * qs well defined for masked keys; an all-zero query row still gives s == 0 everywhere
     const float qs = (row < a.N) ? fmaxf(a.Qs[(size_t)bh * a.N + row], 1e-30f) : 1e-30f;
     const float2 qs2 = make_float2(qs, qs);
-    const uint32_t s_addr = tmem_base + lane_off + TM_S + g * 128;
+    const uint32_t s_addr = tmem_base + lane_off + TM_S + g * 128 + cb;
+    const int pair_bar = 1 + 4 * g + (warp & 3);     // named barrier of the two warps that share these 32 rows
     for (int j = g; j < nblk; j += 2) {
-      const int ring = j % KS_RING;
-      const float2* ks2 = reinterpret_cast<const float2*>(sKs + ring * 128);
-      const int nvalid = min(kTile, a.N - j * kTile);    // < 128 only on the ragged last block
-      const bool ragged = nvalid < kTile;
+      const int n = j >> 1;
+      const int ring = j % KS_RING, slot = j % P_SLOTS, abslot = j % AB_RING;
+      const float2* ks2 = reinterpret_cast<const float2*>(sKs + ring * 128 + cb);
+      const int nvalid = min(kTile, a.N - j * kTile) - cb;   // valid keys of this half; < 64 only on the ragged last block
+      const bool ragged = nvalid < 64;
       mbar_wait(&ks_full[ring], (j / KS_RING) & 1);
-      mbar_wait(&s_full[g], (j >> 1) & 1);
+      mbar_wait(&s_full[g], n & 1);
       tc_fence_after();
-      uint32_t va[32], vb[32];
-      // ---- pass 1: block row max
+      uint32_t va[16], vb[16];
+      // ---- pass 1: block row max over this half
       float mx0 = -INFINITY, mx1 = -INFINITY;
-      tmem_ld32(s_addr, va);
+      tmem_ld16(s_addr, va);
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
         tmem_wait_ld();
-        uint32_t(&cur)[32] = (c & 1) ? vb : va;
-        uint32_t(&nxt)[32] = (c & 1) ? va : vb;
-        tmem_ld32(s_addr + ((c + 1) & 3) * 32, nxt);     // chunk c+1 (after chunk 3: chunk 0 again, for pass 2)
-        if (ragged) chunk_max<true>(cur, ks2 + c * 16, nvalid - c * 32, mx0, mx1);
-        else chunk_max<false>(cur, ks2 + c * 16, 32, mx0, mx1);
+        uint32_t(&cur)[16] = (c & 1) ? vb : va;
+        uint32_t(&nxt)[16] = (c & 1) ? va : vb;
+        tmem_ld16(s_addr + ((c + 1) & 3) * 16, nxt);     // chunk c+1 (after chunk 3: chunk 0 again, for pass 2)
+        if (ragged) chunk_max<true>(cur, ks2 + c * 8, nvalid - c * 16, mx0, mx1);
+        else chunk_max<false>(cur, ks2 + c * 8, 16, mx0, mx1);
       }
-      const float mt = qs * fmaxf(mx0, mx1);             // block row max of s * log2e
-      const float2 nref2 = make_float2(-mt, -mt);
-      // ---- pass 2: P^, row sum, codes -> u8 P tile (aliases S columns [0,32) of this buffer)
+      float tmax = fmaxf(mx0, mx1);
+      float* mxbuf = sMx + ((g * 2 + (n & 1)) * 2) * 128;
+      mxbuf[h * 128 + r] = tmax;
+      bar_sync(pair_bar, 64);
+      tmax = fmaxf(tmax, mxbuf[(h ^ 1) * 128 + r]);
+      const float mt = qs * tmax;                        // block row max of s * log2e
+      const float nref = LOG2_LEVELS - mt;
+      const float2 nref2 = make_float2(nref, nref);
+      mbar_wait(&p_empty[slot], ((j / P_SLOTS) & 1) ^ 1);
+      // ---- pass 2: LEVELS * P^, row sum, codes -> u8 P tile slot
       float2 ls0 = make_float2(0.f, 0.f), ls1 = make_float2(0.f, 0.f);
+      const uint32_t p_addr = tmem_base + lane_off + TM_P + slot * 32 + 16 * h;
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
         tmem_wait_ld();
-        uint32_t(&cur)[32] = (c & 1) ? vb : va;
-        uint32_t(&nxt)[32] = (c & 1) ? va : vb;
-        if (c < 3) tmem_ld32(s_addr + (c + 1) * 32, nxt);
+        uint32_t(&cur)[16] = (c & 1) ? vb : va;
+        uint32_t(&nxt)[16] = (c & 1) ? va : vb;
+        if (c < 3) tmem_ld16(s_addr + (c + 1) * 16, nxt);
+        else { tc_fence_before(); mbar_arrive(&s_empty[g]); }          // this thread is done with the S buffer
         if (DEBUG) {
 #pragma unroll
-          for (int i = 0; i < 32; ++i) a.S_dump[(size_t)r * a.npad + j * kTile + c * 32 + i] = (int32_t)(__uint_as_float(cur[i]) * kAccScale);
+          for (int i = 0; i < 16; ++i)
+            a.S_dump[(size_t)r * a.npad + j * kTile + cb + c * 16 + i] = (int32_t)(__uint_as_float(cur[i]) * kAccScale);
         }
-        uint32_t pw[8];
-        if (ragged) chunk_exp<true, P_MODE>(cur, ks2 + c * 16, nvalid - c * 32, qs2, nref2, ls0, ls1, pw);
-        else chunk_exp<false, P_MODE>(cur, ks2 + c * 16, 32, qs2, nref2, ls0, ls1, pw);
+        uint32_t pw[4];
+        if (ragged) chunk_exp<true>(cur, ks2 + c * 8, nvalid - c * 16, qs2, nref2, ls0, ls1, pw);
+        else chunk_exp<false>(cur, ks2 + c * 8, 16, qs2, nref2, ls0, ls1, pw);
         if (DEBUG) {
 #pragma unroll
-          for (int q = 0; q < 8; ++q) *reinterpret_cast<uint32_t*>(a.P_dump + (size_t)r * a.npad + j * kTile + c * 32 + q * 4) = pw[q];
+          for (int q = 0; q < 4; ++q) *reinterpret_cast<uint32_t*>(a.P_dump + (size_t)r * a.npad + j * kTile + cb + c * 16 + q * 4) = pw[q];
         }
-        tmem_st8(s_addr + c * 8, pw);
+        tmem_st4(p_addr + c * 4, pw);
       }
-      sAB[(j % AB_RING) * 128 + r] = make_float2(mt, (ls0.x + ls0.y) + (ls1.x + ls1.y));
+      sAB[(abslot * 2 + h) * 128 + r] = make_float2(mt, (ls0.x + ls0.y) + (ls1.x + ls1.y));
       tmem_wait_st();
       tc_fence_before();
-      mbar_arrive(&p_full[g]);
-      mbar_arrive(&ab_full[j % AB_RING]);
+      mbar_arrive(&p_full[slot]);
+      mbar_arrive(&ab_full[abslot]);
       mbar_arrive(&ks_empty[ring]);
     }
   } else {
     // ------------------------------------------------------------------ drain: 2 threads per query row of O
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 120;");
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 96;");
     constexpr int DH = D / 2;                      // channels per thread
-    constexpr float INV_LEVELS = kAccScale * (P_MODE == ROTATTN_P_ASYM15 ? 1.f / 15.f : 1.f / 7.f);   // undoes the 2^-18 of the E4M3 code products
-    const int tdr = threadIdx.x - 384;
+    const int tdr = threadIdx.x - 640;
     const int h = tdr >> 7, r = tdr & 127;
     const int row = q0 + r;
     const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
@@ -297,43 +329,43 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     for (int d = 0; d < DH / 2; ++d) o2[d] = make_float2(0.f, 0.f);
     float m_run = -INFINITY, l_run = 0.f;
     for (int j = 0; j < nblk; ++j) {
-      const int b = j & 1;
       // online softmax bookkeeping (L157): m' = max(m, mt); alpha = exp(m - m'); beta = exp(mt - m'); l = alpha l + beta sum(P^)
-      mbar_wait(&ab_full[j % AB_RING], (j / AB_RING) & 1);
-      const float2 ms = sAB[(j % AB_RING) * 128 + r];
-      const float m_new = fmaxf(m_run, ms.x);
+      const int abslot = j % AB_RING;
+      mbar_wait(&ab_full[abslot], (j / AB_RING) & 1);
+      const float2 ms0 = sAB[(abslot * 2 + 0) * 128 + r], ms1 = sAB[(abslot * 2 + 1) * 128 + r];
+      const float m_new = fmaxf(m_run, ms0.x);
       const float alpha = ex2_approx(m_run - m_new);                   // first block: exp2(-inf) = 0
-      const float beta = ex2_approx(ms.x - m_new);
-      l_run = alpha * l_run + beta * ms.y;
+      const float beta = ex2_approx(ms0.x - m_new);
+      l_run = alpha * l_run + beta * (ms0.y + ms1.y);                  // in units of LEVELS (cancels in O/l)
       m_run = m_new;
-      const float cf = beta * INV_LEVELS;
+      const float cf = beta * kAccScale;                               // undoes the 2^-18 of the E4M3 code products
       const float2 c2 = make_float2(cf, cf), a2 = make_float2(alpha, alpha);
       const bool keep = __all_sync(0xffffffffu, alpha == 1.f);         // no new row max in this warp's 32 rows
       const int vring = j % VS_RING;
       mbar_wait(&vs_full[vring], (j / VS_RING) & 1);
       const float2* vsb2 = reinterpret_cast<const float2*>(sVs + vring * D + h * DH);
-      mbar_wait(&pv_full[b], (j >> 1) & 1);
+      mbar_wait(pv_full, j & 1);
       tc_fence_after();
 #pragma unroll
-      for (int cc = 0; cc < DH / 32; ++cc) {
-        uint32_t v[32];
-        tmem_ld32(tmem_base + lane_off + TM_PV + b * 128 + h * DH + cc * 32, v);
+      for (int cc = 0; cc < DH / 16; ++cc) {
+        uint32_t v[16];
+        tmem_ld16(tmem_base + lane_off + TM_PV + h * DH + cc * 16, v);
         tmem_wait_ld();
-        if (cc == DH / 32 - 1) {                                       // PV buffer is in registers now
+        if (cc == DH / 16 - 1) {                                       // PV buffer is in registers now
           tc_fence_before();
-          mbar_arrive(&pv_empty[b]);
+          mbar_arrive(pv_empty);
         }
         if (keep) {
 #pragma unroll
-          for (int d = 0; d < 16; ++d) {
-            const float2 y = fmul2(make_float2(__uint_as_float(v[2 * d]), __uint_as_float(v[2 * d + 1])), vsb2[cc * 16 + d]);
-            o2[cc * 16 + d] = ffma2(y, c2, o2[cc * 16 + d]);           // O += (beta/levels) * pv * Vs[g][d]
+          for (int d = 0; d < 8; ++d) {
+            const float2 y = fmul2(make_float2(__uint_as_float(v[2 * d]), __uint_as_float(v[2 * d + 1])), vsb2[cc * 8 + d]);
+            o2[cc * 8 + d] = ffma2(y, c2, o2[cc * 8 + d]);             // O += beta * pv * Vs[g][d]
           }
         } else {
 #pragma unroll
-          for (int d = 0; d < 16; ++d) {
-            const float2 y = fmul2(make_float2(__uint_as_float(v[2 * d]), __uint_as_float(v[2 * d + 1])), vsb2[cc * 16 + d]);
-            o2[cc * 16 + d] = ffma2(o2[cc * 16 + d], a2, fmul2(y, c2));   // O = alpha O + (beta/levels) * pv * Vs[g][d]
+          for (int d = 0; d < 8; ++d) {
+            const float2 y = fmul2(make_float2(__uint_as_float(v[2 * d]), __uint_as_float(v[2 * d + 1])), vsb2[cc * 8 + d]);
+            o2[cc * 8 + d] = ffma2(o2[cc * 8 + d], a2, fmul2(y, c2));  // O = alpha O + beta * pv * Vs[g][d]
           }
         }
       }
@@ -368,10 +400,10 @@ int launch_variant(const rotattn_params& p, const CUtensorMap& tq, const CUtenso
   constexpr int smem = SmemInt4<D>::TOTAL;
   if (p.p_mode == ROTATTN_P_ASYM15) {
     ROTATTN_CUDA_TRY(cudaFuncSetAttribute(fwd_int4_kernel<D, ROTATTN_P_ASYM15, DEBUG>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    fwd_int4_kernel<D, ROTATTN_P_ASYM15, DEBUG><<<grid, kInt4Threads, smem, cs>>>(tq, tk, tv, a);
+    fwd_int4_kernel<D, ROTATTN_P_ASYM15, DEBUG><<<grid, kFwdThreads, smem, cs>>>(tq, tk, tv, a);
   } else {
     ROTATTN_CUDA_TRY(cudaFuncSetAttribute(fwd_int4_kernel<D, ROTATTN_P_SYM7, DEBUG>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    fwd_int4_kernel<D, ROTATTN_P_SYM7, DEBUG><<<grid, kInt4Threads, smem, cs>>>(tq, tk, tv, a);
+    fwd_int4_kernel<D, ROTATTN_P_SYM7, DEBUG><<<grid, kFwdThreads, smem, cs>>>(tq, tk, tv, a);
   }
   ROTATTN_CUDA_TRY(cudaGetLastError());
   return ROTATTN_OK;
