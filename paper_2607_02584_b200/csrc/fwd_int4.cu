@@ -2,20 +2,23 @@
 // bytes, see fwd_int4.cuh), row-block P normaliser.
 //
 // One CTA = one 128-row query tile of one (b,h); 28 warps, warp-specialised:
-//   warp 0        TMA producer : Q tile once, K tiles (4-stage ring) and V^T tiles (3-stage ring)
-//   warp 1        MMA issuer   : S = Q K^T (codes x codes, exact, TMEM), P~V (P codes from TMEM x V codes, TMEM)
-//   warp 2        TMEM allocator, then V-scale loader (Vs[g][:] -> shared ring)
-//   warp 3        K-scale loader (Ks[j] * 2^18 log2e/sqrt(D) -> shared ring)
-//   warps 4-11    softmax group 0: even KV blocks; warps 4-7 own keys [0,64) of the block, warps 8-11 keys [64,128)
-//   warps 12-19   softmax group 1: odd KV blocks, same split  (two threads per query row and block)
-//   warps 20-27   drain: 2 threads per query row (D/2 channels each): online-softmax bookkeeping (m, l, alpha, beta),
+//   warps 0-7     softmax group 0: even KV blocks; warps 0-3 own keys [0,64) of the block, warps 4-7 keys [64,128)
+//   warps 8-15    softmax group 1: odd KV blocks, same split  (two threads per query row and block)
+//   warps 16-23   drain: 2 threads per query row (D/2 channels each): online-softmax bookkeeping (m, l, alpha, beta),
 //                 P~V block -> fp32 O registers, epilogue O/l
+//   warp 24       TMEM allocator, then scale loader (Ks[j] * 2^18 log2e/sqrt(D) and Vs[g][:] -> shared rings)
+//   warp 25       TMA producer  : Q tile once, K tiles and V^T tiles (4-stage rings)
+//   warp 26       MMA issuer 2  : P~V (P codes from TMEM x V codes, TMEM)
+//   warp 27       MMA issuer 1  : S = Q K^T (codes x codes, exact, TMEM)
 // With the row-block normaliser (reading 13) the codes of block j depend only on block j, so the two softmax
 // groups work on different blocks concurrently and the running max lives in the drain threads.  Each softmax thread
-// makes two passes over its half row of S in tensor memory (pass 1: block row max, exchanged with the partner thread
-// through shared memory; pass 2: exp2 / row sum / codes) in 16-column chunks.
-// TMEM (512 columns): S[2] at 0/128, PV at 256, four P-code slots of 32 columns at 384.  P has its own slots so that
-// an S buffer is released as soon as pass 2 has read it (S(j+2) is issued before P~V(j), hiding the MMA latency).
+// makes two passes over its half row of S in tensor memory in 16-column chunks: pass 1 scales by the key scales, writes
+// t back over S and takes the block row max (exchanged with the partner thread through shared memory); pass 2 reads t:
+// exp2 / row sum / codes.
+// TMEM (512 columns): S[2] at 0/128, two P-code slots of 32 columns at 256, three half-width (D/2 channels) P~V
+// accumulators of 64 columns at 320 used in rotation (half k = 2j+h -> buffer k % 3), so that the P~V MMAs run ahead of
+// the drain instead of alternating with it.  P has its own slots so that an S buffer is released as soon as pass 2 has
+// read it (S(j+2) is issued before P~V(j), hiding the MMA latency).
 // The per-block drain is forced by the method: beta (row, block) and Vs (channel, block) change every KV block
 // (PAPER.md:L157 online softmax, L190 per-group V scales), so P~V cannot accumulate across blocks in tensor memory.
 #include <cmath>
@@ -25,12 +28,17 @@
 namespace rotattn {
 
 constexpr int kFwdThreads = 896;
+// Warp roles.  Within an SM sub-partition the scheduler favours the highest warp id among the eligible warps, so the
+// latency-critical single-thread roles (MMA issue, TMA) get the highest ids and the throughput roles the lowest.
+constexpr int kWarpScale = 24, kWarpTma = 25, kWarpMmaPV = 26, kWarpMmaS = 27;
 constexpr int K_STAGES = 4;
-constexpr int V_STAGES = 3;
-constexpr int P_SLOTS = 4;
+constexpr int V_STAGES = 4;
+constexpr int P_SLOTS = 2;
+constexpr int PV_BUFS = 3;       // half-width (D/2 channel) P~V accumulators in rotation
 constexpr int AB_RING = 8;
 constexpr int KS_RING = 4;
 constexpr int VS_RING = 4;
+static_assert(K_STAGES == 4 && V_STAGES == 4 && P_SLOTS == 2 && KS_RING == VS_RING, "ring sizes are tied together by the shared completion barriers");
 
 template <int D>
 struct SmemInt4 {
@@ -45,44 +53,38 @@ struct SmemInt4 {
   static constexpr int OFF_AB = OFF_VS + VS_RING * D * 4;             // float2 [AB_RING][2 halves][128]  (block max, half-row sum)
   static constexpr int OFF_MX = OFF_AB + AB_RING * 2 * 128 * 8;       // float [2 groups][2 parities][2 halves][128]
   static constexpr int OFF_BAR = OFF_MX + 2 * 2 * 2 * 128 * 4;        // mbarriers
-  static constexpr int NBAR = 1 + 2 * K_STAGES + 2 * V_STAGES + 2 + 2 + 2 * P_SLOTS + 2 + AB_RING + 2 * KS_RING + 2 * VS_RING;
+  static constexpr int NBAR = 1 + 2 * K_STAGES + 2 * V_STAGES + 2 + P_SLOTS + 2 * PV_BUFS + AB_RING + 2 * KS_RING + 2 * VS_RING;
   static constexpr int OFF_TMEM = OFF_BAR + NBAR * 8;
   static constexpr int TOTAL = OFF_TMEM + 16;
 };
 
 // ---- per-chunk element-wise work of the softmax threads (16 S columns of one query row) -------------------------
-// t = S * (Ks_j * 2^18 log2e/sqrt(D)) (the query scale Qs_i > 0 is applied after the max); keys >= N are masked to -inf.
+// Pass 1: t = S * (Ks_j * 2^18 log2e/sqrt(D)) (the query scale Qs_i > 0 is applied after the max); keys >= N are masked
+// to -inf.  t overwrites S in tensor memory so that pass 2 needs neither the key scales nor the mask.
 template <bool MASK>
-__device__ __forceinline__ void chunk_scale(const uint32_t (&v)[16], const float2* ks2, int nvalid_rel, float2 (&t2)[8]) {
+__device__ __forceinline__ void chunk_scale_max(const uint32_t (&v)[16], const float2* ks2, int nvalid_rel, uint32_t (&t)[16],
+                                                float& mx0, float& mx1) {
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
-    t2[i] = fmul2(make_float2(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1])), ks2[i]);
+    float2 t2 = fmul2(make_float2(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1])), ks2[i]);
     if (MASK) {
-      if (2 * i >= nvalid_rel) t2[i].x = -INFINITY;
-      if (2 * i + 1 >= nvalid_rel) t2[i].y = -INFINITY;
+      if (2 * i >= nvalid_rel) t2.x = -INFINITY;
+      if (2 * i + 1 >= nvalid_rel) t2.y = -INFINITY;
     }
+    if (i & 1) mx1 = fmax3(mx1, t2.x, t2.y); else mx0 = fmax3(mx0, t2.x, t2.y);
+    t[2 * i] = __float_as_uint(t2.x);
+    t[2 * i + 1] = __float_as_uint(t2.y);
   }
 }
 
-template <bool MASK>
-__device__ __forceinline__ void chunk_max(const uint32_t (&v)[16], const float2* ks2, int nvalid_rel, float& mx0, float& mx1) {
-  float2 t2[8];
-  chunk_scale<MASK>(v, ks2, nvalid_rel, t2);
-#pragma unroll
-  for (int i = 0; i < 8; i += 2) { mx0 = fmax3(mx0, t2[i].x, t2[i].y); mx1 = fmax3(mx1, t2[i + 1].x, t2[i + 1].y); }
-}
-
-// LEVELS * P^ = exp2(t * Qs_i - mt + log2(LEVELS)); codes u = rne(LEVELS * P^) taken from the low byte of
+// Pass 2: LEVELS * P^ = exp2(t * Qs_i - mt + log2(LEVELS)); codes u = rne(LEVELS * P^) taken from the low byte of
 // (LEVELS * P^) + 1.5 * 2^23 (Eq.12 L166-168 with the fixed scale 15 / Eq.11 L161 with 7); four codes per TMEM column.
-template <bool MASK>
-__device__ __forceinline__ void chunk_exp(const uint32_t (&v)[16], const float2* ks2, int nvalid_rel, float2 qs2, float2 nref2,
-                                          float2& ls0, float2& ls1, uint32_t (&pw)[4]) {
+__device__ __forceinline__ void chunk_exp(const uint32_t (&t)[16], float2 qs2, float2 nref2, float2& ls0, float2& ls1, uint32_t (&pw)[4]) {
   const float2 magic2 = make_float2(12582912.f, 12582912.f);
-  float2 t2[8];
-  chunk_scale<MASK>(v, ks2, nvalid_rel, t2);
 #pragma unroll
   for (int g = 0; g < 4; ++g) {
-    const float2 e0 = ffma2(t2[2 * g], qs2, nref2), e1 = ffma2(t2[2 * g + 1], qs2, nref2);
+    const float2 e0 = ffma2(make_float2(__uint_as_float(t[4 * g]), __uint_as_float(t[4 * g + 1])), qs2, nref2);
+    const float2 e1 = ffma2(make_float2(__uint_as_float(t[4 * g + 2]), __uint_as_float(t[4 * g + 3])), qs2, nref2);
     const float2 p0 = make_float2(ex2_approx(e0.x), ex2_approx(e0.y));
     const float2 p1 = make_float2(ex2_approx(e1.x), ex2_approx(e1.y));
     ls0 = fadd2(ls0, p0);
@@ -109,24 +111,23 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   float* sMx = (float*)(smem + L::OFF_MX);
   uint64_t* bars = (uint64_t*)(smem + L::OFF_BAR);
   uint64_t* q_full = bars;
-  uint64_t* k_full = q_full + 1;
-  uint64_t* k_empty = k_full + K_STAGES;
-  uint64_t* v_full = k_empty + K_STAGES;
-  uint64_t* v_empty = v_full + V_STAGES;
-  uint64_t* s_full = v_empty + V_STAGES;      // [2] MMA -> softmax group (buffer b belongs to group b)
-  uint64_t* s_empty = s_full + 2;             // [2] softmax group -> MMA (count 256): S buffer has been read
+  uint64_t* k_full = q_full + 1;              // [K_STAGES] TMA -> MMA
+  uint64_t* v_full = k_full + K_STAGES;       // [V_STAGES] TMA -> MMA
+  uint64_t* s_done = v_full + V_STAGES;       // [K_STAGES] S(m) complete: -> softmax group m & 1 (S ready), -> TMA (K stage free)
+  uint64_t* s_empty = s_done + K_STAGES;      // [2] softmax group -> MMA (count 256): S buffer has been read
   uint64_t* p_full = s_empty + 2;             // [P_SLOTS] softmax group -> MMA (count 256)
-  uint64_t* p_empty = p_full + P_SLOTS;       // [P_SLOTS] MMA -> softmax: P~V has consumed the slot
-  uint64_t* pv_full = p_empty + P_SLOTS;      // MMA -> drain
-  uint64_t* pv_empty = pv_full + 1;           // drain -> MMA (count 256)
-  uint64_t* ab_full = pv_empty + 1;           // [AB_RING] softmax -> drain (count 256)
+  uint64_t* pv_done = p_full + P_SLOTS;       // [V_STAGES] both halves of P~V(j) complete: -> softmax (P slot free), TMA (V stage free)
+  uint64_t* pvh_done = pv_done + V_STAGES;    // [PV_BUFS] half k = 2j+h of P~V complete -> drain warps of channel half h
+  uint64_t* pvh_empty = pvh_done + PV_BUFS;   // [PV_BUFS] drain -> MMA (count 128): half buffer is in registers
+  uint64_t* ab_full = pvh_empty + PV_BUFS;    // [AB_RING] softmax -> drain (count 256)
   uint64_t* ks_full = ab_full + AB_RING;      // [KS_RING] loader -> softmax (count 32)
   uint64_t* ks_empty = ks_full + KS_RING;     // [KS_RING] softmax -> loader (count 256)
   uint64_t* vs_full = ks_empty + KS_RING;     // [VS_RING] loader -> drain (count 32)
   uint64_t* vs_empty = vs_full + VS_RING;     // [VS_RING] drain -> loader (count 256)
   uint32_t* tmem_slot = (uint32_t*)(smem + L::OFF_TMEM);
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);   // warp-uniform (kept in a uniform register)
+  const int lane = threadIdx.x & 31;
   const int qtile = DEBUG ? a.dbg_qtile : blockIdx.x;
   const int bh = DEBUG ? a.dbg_bh : (a.head_sel ? a.head_sel[blockIdx.y] : (int)blockIdx.y);
   const int q0 = qtile * kTile;
@@ -135,117 +136,140 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   if (threadIdx.x == 0) {
     if (smem_u32(smem) & 1023u) __trap();     // SWIZZLE_128B operand tiles need 1024-byte alignment
     mbar_init(q_full, 1);
-    for (int i = 0; i < K_STAGES; ++i) { mbar_init(&k_full[i], 1); mbar_init(&k_empty[i], 1); }
-    for (int i = 0; i < V_STAGES; ++i) { mbar_init(&v_full[i], 1); mbar_init(&v_empty[i], 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(&s_full[i], 1); mbar_init(&s_empty[i], 256); }
-    for (int i = 0; i < P_SLOTS; ++i) { mbar_init(&p_full[i], 256); mbar_init(&p_empty[i], 1); }
-    mbar_init(pv_full, 1); mbar_init(pv_empty, 256);
+    for (int i = 0; i < K_STAGES; ++i) { mbar_init(&k_full[i], 1); mbar_init(&s_done[i], 1); }
+    for (int i = 0; i < V_STAGES; ++i) mbar_init(&v_full[i], 1);
+    for (int i = 0; i < 2; ++i) mbar_init(&s_empty[i], 256);
+    for (int i = 0; i < P_SLOTS; ++i) mbar_init(&p_full[i], 256);
+    for (int i = 0; i < V_STAGES; ++i) mbar_init(&pv_done[i], 1);
+    for (int i = 0; i < PV_BUFS; ++i) { mbar_init(&pvh_done[i], 1); mbar_init(&pvh_empty[i], 128); }
     for (int i = 0; i < AB_RING; ++i) mbar_init(&ab_full[i], 256);
     for (int i = 0; i < KS_RING; ++i) { mbar_init(&ks_full[i], 32); mbar_init(&ks_empty[i], 256); }
     for (int i = 0; i < VS_RING; ++i) { mbar_init(&vs_full[i], 32); mbar_init(&vs_empty[i], 256); }
     fence_mbar_init();
   }
-  if (warp == 2) tmem_alloc(tmem_slot, 512);
+  if (warp == kWarpScale) tmem_alloc(tmem_slot, 512);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
-  constexpr uint32_t TM_S = 0, TM_PV = 256, TM_P = 384;
+  constexpr uint32_t TM_S = 0, TM_P = 256, TM_PV = 320;     // S[2] x 128 | P[2] x 32 | PV half buffers [3] x 64
 
   // register pool of the CTA = 896 x 72; after redistribution 128 x 24 + 512 x 72 + 256 x 96 = 64512 (exactly the pool)
-  if (warp < 4) {
+  if (warp >= 24) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
-    if (warp == 0) {
+    // The single-thread roles keep warp-uniform control flow (every lane waits; one elected lane issues), so that the
+    // TMA / MMA operands stay in uniform registers.
+    if (warp == kWarpTma) {
       // ---------------------------------------------------------------- TMA producer
-      if (lane == 0) {
+      if (elect_one()) {
         tma_prefetch_desc(&tmQ); tma_prefetch_desc(&tmK); tma_prefetch_desc(&tmV);
         mbar_arrive_expect_tx(q_full, L::Q_BYTES);
         tma_load_3d(sQ, &tmQ, q_full, 0, q0, bh);
-        auto load_k = [&](int m) {
+      }
+      __syncwarp();
+      for (int i = 0; i < nblk + 2; ++i) {
+        const int m = i, j = i - 2;                                      // K runs two blocks ahead of V
+        if (m < nblk) {
           const int s = m % K_STAGES;
-          mbar_wait(&k_empty[s], ((m / K_STAGES) & 1) ^ 1);
-          mbar_arrive_expect_tx(&k_full[s], L::K_BYTES);
-          tma_load_3d(sK + s * L::K_BYTES, &tmK, &k_full[s], 0, m * kTile, bh);
-        };
-        load_k(0);
-        if (nblk > 1) load_k(1);
-        for (int j = 0; j < nblk; ++j) {
-          if (j + 2 < nblk) load_k(j + 2);
+          mbar_wait(&s_done[s], ((m / K_STAGES) & 1) ^ 1);               // S(m-4) has consumed this K stage
+          if (elect_one()) {
+            mbar_arrive_expect_tx(&k_full[s], L::K_BYTES);
+            tma_load_3d(sK + s * L::K_BYTES, &tmK, &k_full[s], 0, m * kTile, bh);
+          }
+          __syncwarp();
+        }
+        if (j >= 0) {
           const int s = j % V_STAGES;
-          mbar_wait(&v_empty[s], ((j / V_STAGES) & 1) ^ 1);
-          mbar_arrive_expect_tx(&v_full[s], L::V_BYTES);
-          tma_load_3d(sV + s * L::V_BYTES, &tmV, &v_full[s], j * kTile, 0, bh);
+          mbar_wait(&pv_done[s], ((j / V_STAGES) & 1) ^ 1);              // P~V(j-4) has consumed this V stage
+          if (elect_one()) {
+            mbar_arrive_expect_tx(&v_full[s], L::V_BYTES);
+            tma_load_3d(sV + s * L::V_BYTES, &tmV, &v_full[s], j * kTile, 0, bh);
+          }
+          __syncwarp();
         }
       }
-    } else if (warp == 1) {
-      // ---------------------------------------------------------------- MMA issuer
-      if (lane == 0) {
-        constexpr uint32_t idesc_s = umma_idesc(1, 0, 0, 128, 128);      // f32 <- e4m3 x e4m3 (integer codes * 2^-9)
-        constexpr uint32_t idesc_pv = umma_idesc(1, 0, 0, 128, D);
-        constexpr int KSTEPS_S = D / 32;                                 // D=64 rows are zero-padded to 128 B
-        const uint64_t qd = umma_desc_k128(smem_u32(sQ));
-        auto issue_s = [&](int m) {                                      // S(m) -> buffer m & 1
-          const int st = m % K_STAGES, b = m & 1;
-          mbar_wait(&k_full[st], (m / K_STAGES) & 1);
-          if (m >= 2) mbar_wait(&s_empty[b], ((m >> 1) - 1) & 1);        // softmax has read S(m-2) out of this buffer
-          tc_fence_after();
+    } else if (warp == kWarpMmaS) {
+      // ---------------------------------------------------------------- MMA issuer 1: S(m) = Q K(m)^T -> buffer m & 1
+      constexpr uint32_t idesc_s = umma_idesc(1, 0, 0, 128, 128);        // f32 <- e4m3 x e4m3 (integer codes * 2^-9)
+      constexpr int KSTEPS_S = D / 32;                                   // D=64 rows are zero-padded to 128 B
+      const uint64_t qd = umma_desc_k128(smem_u32(sQ));
+      mbar_wait(q_full, 0);
+      for (int m = 0; m < nblk; ++m) {
+        const int st = m % K_STAGES, b = m & 1;
+        ROTATTN_STAMP(m, 4);
+        mbar_wait(&k_full[st], (m / K_STAGES) & 1);
+        ROTATTN_STAMP(m, 5);
+        if (m >= 2) mbar_wait(&s_empty[b], ((m >> 1) - 1) & 1);          // softmax has read S(m-2) out of this buffer
+        tc_fence_after();
+        ROTATTN_STAMP(m, 6);
+        if (elect_one()) {
           const uint64_t kd = umma_desc_k128(smem_u32(sK + st * L::K_BYTES));
 #pragma unroll
           for (int k = 0; k < KSTEPS_S; ++k)
             mma_ss<MmaKind::F8F6F4>(tmem_base + TM_S + b * 128, qd + 2 * k, kd + 2 * k, idesc_s, k != 0);
-          tc_commit(&k_empty[st]);
-          tc_commit(&s_full[b]);
-        };
-        mbar_wait(q_full, 0);
-        issue_s(0);
-        if (nblk > 1) issue_s(1);
-        for (int j = 0; j < nblk; ++j) {
-          if (j + 2 < nblk) issue_s(j + 2);                              // goes ahead of P~V(j): only needs S(j) to be read
-          const int slot = j % P_SLOTS, vst = j % V_STAGES;
-          mbar_wait(&p_full[slot], (j / P_SLOTS) & 1);
-          mbar_wait(&v_full[vst], (j / V_STAGES) & 1);
-          mbar_wait(pv_empty, (j & 1) ^ 1);
-          tc_fence_after();
-          const uint64_t vd = umma_desc_k128(smem_u32(sV + vst * L::V_BYTES));
-#pragma unroll
-          for (int k = 0; k < 4; ++k)
-            mma_ts<MmaKind::F8F6F4>(tmem_base + TM_PV, tmem_base + TM_P + slot * 32 + 8 * k, vd + 2 * k, idesc_pv, k != 0);
-          tc_commit(&v_empty[vst]);
-          tc_commit(&p_empty[slot]);
-          tc_commit(pv_full);
+          tc_commit(&s_done[st]);                                        // -> softmax group (S ready) and TMA (K stage free)
         }
+        __syncwarp();
+        ROTATTN_STAMP(m, 0);
       }
-    } else if (warp == 2) {
-      // ---------------------------------------------------------------- V-scale loader
-      const float* vsrc = a.Vs + (size_t)bh * nblk * D;
+    } else if (warp == kWarpMmaPV) {
+      // ---------------------------------------------------------------- MMA issuer 2: PV = P~(j) V(j)
+      constexpr uint32_t idesc_pv = umma_idesc(1, 0, 0, 128, D / 2);
+      int buf = 0; uint32_t bpar = 1;                                    // rotation state of half k = 2j + h: k % 3, ((k / 3) & 1) ^ 1
       for (int j = 0; j < nblk; ++j) {
-        const int s = j % VS_RING;
-        mbar_wait(&vs_empty[s], ((j / VS_RING) & 1) ^ 1);
+        const int slot = j % P_SLOTS, vst = j % V_STAGES;
+        mbar_wait(&v_full[vst], (j / V_STAGES) & 1);
+        mbar_wait(&p_full[slot], (j / P_SLOTS) & 1);
+        ROTATTN_STAMP(j, 1);
 #pragma unroll
-        for (int i = 0; i < D / 32; ++i) sVs[s * D + i * 32 + lane] = vsrc[(size_t)j * D + i * 32 + lane];
-        mbar_arrive(&vs_full[s]);
+        for (int h = 0; h < 2; ++h) {
+          mbar_wait(&pvh_empty[buf], bpar);                              // drain has read half k-3 out of this buffer
+          tc_fence_after();
+          if (h == 0) ROTATTN_STAMP(j, 3);
+          if (elect_one()) {
+            // V^T tile: channel half h starts D/2 rows (= D/2 * 128 B, whole 1024-byte swizzle atoms) into the tile
+            const uint64_t vd = umma_desc_k128(smem_u32(sV + vst * L::V_BYTES + h * (D / 2) * 128));
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+              mma_ts<MmaKind::F8F6F4>(tmem_base + TM_PV + buf * 64, tmem_base + TM_P + slot * 32 + 8 * k, vd + 2 * k, idesc_pv, k != 0);
+            tc_commit(&pvh_done[buf]);                                   // -> drain warps of this channel half
+            if (h == 1) tc_commit(&pv_done[vst]);                        // -> softmax (P slot free), TMA (V stage free)
+          }
+          __syncwarp();
+          if (++buf == PV_BUFS) { buf = 0; bpar ^= 1; }
+        }
+        ROTATTN_STAMP(j, 9);
       }
     } else {
-      // ---------------------------------------------------------------- K-scale loader: Ks_j * 2^18 log2e/sqrt(D)
+      // ---------------------------------------------------------------- scale loader: Ks_j * 2^18 log2e/sqrt(D), Vs[g][:]
       const float* ksrc = a.Ks + (size_t)bh * a.N;
+      const float* vsrc = a.Vs + (size_t)bh * nblk * D;
       for (int j = 0; j < nblk; ++j) {
         const int s = j % KS_RING;
-        mbar_wait(&ks_empty[s], ((j / KS_RING) & 1) ^ 1);
+        float kv[4], vv[D / 32];
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
           const int kj = j * kTile + i * 32 + lane;
-          sKs[s * 128 + i * 32 + lane] = (kj < a.N) ? ksrc[kj] * a.scale_log2 : 0.f;
+          kv[i] = (kj < a.N) ? ksrc[kj] * a.scale_log2 : 0.f;
         }
+#pragma unroll
+        for (int i = 0; i < D / 32; ++i) vv[i] = vsrc[(size_t)j * D + i * 32 + lane];
+        mbar_wait(&ks_empty[s], ((j / KS_RING) & 1) ^ 1);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) sKs[s * 128 + i * 32 + lane] = kv[i];
         mbar_arrive(&ks_full[s]);
+        mbar_wait(&vs_empty[s], ((j / VS_RING) & 1) ^ 1);
+#pragma unroll
+        for (int i = 0; i < D / 32; ++i) sVs[s * D + i * 32 + lane] = vv[i];
+        mbar_arrive(&vs_full[s]);
       }
     }
-  } else if (warp < 20) {
+  } else if (warp < 16) {
     // ------------------------------------------------------------------ softmax groups: 0 = even blocks, 1 = odd blocks
     constexpr float LOG2_LEVELS = P_MODE == ROTATTN_P_ASYM15 ? 3.9068905956085187f : 2.8073549220576042f;
-    const int tsm = threadIdx.x - 128;
-    const int g = tsm >> 8;                          // group index = S buffer index
-    const int h = (tsm >> 7) & 1;                    // which 64 keys of the block
-    const int r = tsm & 127;
+    const int g = warp >> 3;                         // group index = S buffer index
+    const int h = (warp >> 2) & 1;                   // which 64 keys of the block
+    const int r = (warp & 3) * 32 + lane;
     const int row = q0 + r;
     const int cb = 64 * h;
     const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
@@ -261,10 +285,11 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       const int nvalid = min(kTile, a.N - j * kTile) - cb;   // valid keys of this half; < 64 only on the ragged last block
       const bool ragged = nvalid < 64;
       mbar_wait(&ks_full[ring], (j / KS_RING) & 1);
-      mbar_wait(&s_full[g], n & 1);
+      mbar_wait(&s_done[j % K_STAGES], (j / K_STAGES) & 1);
       tc_fence_after();
-      uint32_t va[16], vb[16];
-      // ---- pass 1: block row max over this half
+      ROTATTN_STAMP(j, 0);
+      uint32_t va[16], vb[16], tt[16];
+      // ---- pass 1: t = S * ks (written back over S), block row max over this half
       float mx0 = -INFINITY, mx1 = -INFINITY;
       tmem_ld16(s_addr, va);
 #pragma unroll
@@ -272,19 +297,34 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         tmem_wait_ld();
         uint32_t(&cur)[16] = (c & 1) ? vb : va;
         uint32_t(&nxt)[16] = (c & 1) ? va : vb;
-        tmem_ld16(s_addr + ((c + 1) & 3) * 16, nxt);     // chunk c+1 (after chunk 3: chunk 0 again, for pass 2)
-        if (ragged) chunk_max<true>(cur, ks2 + c * 8, nvalid - c * 16, mx0, mx1);
-        else chunk_max<false>(cur, ks2 + c * 8, 16, mx0, mx1);
+        if (c < 3) tmem_ld16(s_addr + (c + 1) * 16, nxt);
+        if (DEBUG) {
+#pragma unroll
+          for (int i = 0; i < 16; ++i)
+            a.S_dump[(size_t)r * a.npad + j * kTile + cb + c * 16 + i] = (int32_t)(__uint_as_float(cur[i]) * kAccScale);
+        }
+#if defined(ROTATTN_ABL) && ROTATTN_ABL == 3      // development ablation: no pass-1 arithmetic / write-back
+        mx0 = fmaxf(mx0, __uint_as_float(cur[0]));
+#else
+        if (ragged) chunk_scale_max<true>(cur, ks2 + c * 8, nvalid - c * 16, tt, mx0, mx1);
+        else chunk_scale_max<false>(cur, ks2 + c * 8, 16, tt, mx0, mx1);
+        tmem_st16(s_addr + c * 16, tt);
+#endif
       }
+      ROTATTN_STAMP(j, 1);
       float tmax = fmaxf(mx0, mx1);
       float* mxbuf = sMx + ((g * 2 + (n & 1)) * 2) * 128;
       mxbuf[h * 128 + r] = tmax;
+      mbar_arrive(&ks_empty[ring]);
+      tmem_wait_st();
+      tmem_ld16(s_addr, va);                             // chunk 0 of t, in flight across the max exchange
       bar_sync(pair_bar, 64);
       tmax = fmaxf(tmax, mxbuf[(h ^ 1) * 128 + r]);
       const float mt = qs * tmax;                        // block row max of s * log2e
       const float nref = LOG2_LEVELS - mt;
       const float2 nref2 = make_float2(nref, nref);
-      mbar_wait(&p_empty[slot], ((j / P_SLOTS) & 1) ^ 1);
+      if (j >= P_SLOTS) mbar_wait(&pv_done[(j - P_SLOTS) % V_STAGES], ((j - P_SLOTS) / V_STAGES) & 1);   // P~V(j-2) has consumed this P slot
+      ROTATTN_STAMP(j, 2);
       // ---- pass 2: LEVELS * P^, row sum, codes -> u8 P tile slot
       float2 ls0 = make_float2(0.f, 0.f), ls1 = make_float2(0.f, 0.f);
       const uint32_t p_addr = tmem_base + lane_off + TM_P + slot * 32 + 16 * h;
@@ -295,14 +335,8 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         uint32_t(&nxt)[16] = (c & 1) ? va : vb;
         if (c < 3) tmem_ld16(s_addr + (c + 1) * 16, nxt);
         else { tc_fence_before(); mbar_arrive(&s_empty[g]); }          // this thread is done with the S buffer
-        if (DEBUG) {
-#pragma unroll
-          for (int i = 0; i < 16; ++i)
-            a.S_dump[(size_t)r * a.npad + j * kTile + cb + c * 16 + i] = (int32_t)(__uint_as_float(cur[i]) * kAccScale);
-        }
         uint32_t pw[4];
-        if (ragged) chunk_exp<true>(cur, ks2 + c * 8, nvalid - c * 16, qs2, nref2, ls0, ls1, pw);
-        else chunk_exp<false>(cur, ks2 + c * 8, 16, qs2, nref2, ls0, ls1, pw);
+        chunk_exp(cur, qs2, nref2, ls0, ls1, pw);
         if (DEBUG) {
 #pragma unroll
           for (int q = 0; q < 4; ++q) *reinterpret_cast<uint32_t*>(a.P_dump + (size_t)r * a.npad + j * kTile + cb + c * 16 + q * 4) = pw[q];
@@ -310,28 +344,31 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         tmem_st4(p_addr + c * 4, pw);
       }
       sAB[(abslot * 2 + h) * 128 + r] = make_float2(mt, (ls0.x + ls0.y) + (ls1.x + ls1.y));
+      ROTATTN_STAMP(j, 3);
       tmem_wait_st();
       tc_fence_before();
       mbar_arrive(&p_full[slot]);
+      ROTATTN_STAMP(j, 4);
       mbar_arrive(&ab_full[abslot]);
-      mbar_arrive(&ks_empty[ring]);
     }
   } else {
     // ------------------------------------------------------------------ drain: 2 threads per query row of O
     asm volatile("setmaxnreg.inc.sync.aligned.u32 96;");
     constexpr int DH = D / 2;                      // channels per thread
-    const int tdr = threadIdx.x - 640;
-    const int h = tdr >> 7, r = tdr & 127;
+    const int h = (warp >> 2) & 1, r = (warp & 3) * 32 + lane;
     const int row = q0 + r;
     const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
     float2 o2[DH / 2];
 #pragma unroll
     for (int d = 0; d < DH / 2; ++d) o2[d] = make_float2(0.f, 0.f);
     float m_run = -INFINITY, l_run = 0.f;
+    int buf = h; uint32_t bpar = 0;                  // rotation state of half k = 2j + h: k % 3, (k / 3) & 1
     for (int j = 0; j < nblk; ++j) {
       // online softmax bookkeeping (L157): m' = max(m, mt); alpha = exp(m - m'); beta = exp(mt - m'); l = alpha l + beta sum(P^)
       const int abslot = j % AB_RING;
+      ROTATTN_STAMP(j, 0);
       mbar_wait(&ab_full[abslot], (j / AB_RING) & 1);
+      ROTATTN_STAMP(j, 1);
       const float2 ms0 = sAB[(abslot * 2 + 0) * 128 + r], ms1 = sAB[(abslot * 2 + 1) * 128 + r];
       const float m_new = fmaxf(m_run, ms0.x);
       const float alpha = ex2_approx(m_run - m_new);                   // first block: exp2(-inf) = 0
@@ -344,24 +381,36 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       const int vring = j % VS_RING;
       mbar_wait(&vs_full[vring], (j / VS_RING) & 1);
       const float2* vsb2 = reinterpret_cast<const float2*>(sVs + vring * D + h * DH);
-      mbar_wait(pv_full, j & 1);
+      mbar_wait(&pvh_done[buf], bpar);
       tc_fence_after();
+      ROTATTN_STAMP(j, 2);
 #pragma unroll
       for (int cc = 0; cc < DH / 16; ++cc) {
         uint32_t v[16];
-        tmem_ld16(tmem_base + lane_off + TM_PV + h * DH + cc * 16, v);
+        tmem_ld16(tmem_base + lane_off + TM_PV + buf * 64 + cc * 16, v);
         tmem_wait_ld();
+        ROTATTN_STAMP(j, 4 + cc);
         if (cc == DH / 16 - 1) {                                       // PV buffer is in registers now
           tc_fence_before();
-          mbar_arrive(pv_empty);
+          mbar_arrive(&pvh_empty[buf]);
         }
+#if defined(ROTATTN_ABL) && ROTATTN_ABL == 2      // development ablation: no drain arithmetic
+        o2[cc].x += __uint_as_float(v[0]);
+        if (false) {
+#else
         if (keep) {
+#endif
 #pragma unroll
           for (int d = 0; d < 8; ++d) {
             const float2 y = fmul2(make_float2(__uint_as_float(v[2 * d]), __uint_as_float(v[2 * d + 1])), vsb2[cc * 8 + d]);
             o2[cc * 8 + d] = ffma2(y, c2, o2[cc * 8 + d]);             // O += beta * pv * Vs[g][d]
           }
-        } else {
+        }
+#if defined(ROTATTN_ABL) && ROTATTN_ABL == 2
+        else if (false) {
+#else
+        else {
+#endif
 #pragma unroll
           for (int d = 0; d < 8; ++d) {
             const float2 y = fmul2(make_float2(__uint_as_float(v[2 * d]), __uint_as_float(v[2 * d + 1])), vsb2[cc * 8 + d]);
@@ -370,6 +419,9 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         }
       }
       mbar_arrive(&vs_empty[vring]);
+      buf += 2;                                       // k -> k + 2
+      if (buf >= PV_BUFS) { buf -= PV_BUFS; bpar ^= 1; }
+      ROTATTN_STAMP(j, 3);
     }
     const float inv_l = 1.f / l_run;
     if (row < a.N) {
@@ -385,12 +437,17 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 2) tmem_dealloc(tmem_base, 512);
+  if (warp == kWarpScale) tmem_dealloc(tmem_base, 512);
 }
 
 }  // namespace rotattn
 
 using namespace rotattn;
+
+#ifdef ROTATTN_TRACE
+static long long* g_rotattn_trace = nullptr;
+extern "C" void rotattn_set_trace(long long* p) { g_rotattn_trace = p; }
+#endif
 
 namespace {
 
@@ -444,6 +501,9 @@ int fwd_int4_common(const rotattn_params* p, const uint8_t* Q4, const float* Qs,
   a.S_dump = S_dump; a.P_dump = P_dump;
   a.N = p->N; a.nblk = nblk; a.npad = ws.npad; a.dbg_bh = bh; a.dbg_qtile = q_tile;
   a.scale_log2 = (float)(1.4426950408889634 / std::sqrt((double)p->D) * (double)kAccScale);   // S arrives as acc * 2^-18
+#ifdef ROTATTN_TRACE
+  a.trace = g_rotattn_trace;
+#endif
   dim3 grid(debug ? 1 : nblk, debug ? 1 : (head_sel ? n_sel : BH));
   if (p->p_norm == ROTATTN_NORM_RUNNING) return launch_fwd_int4_sync(*p, tq, tk, tv, a, grid, debug, cs);
   if (p->D == 128) return debug ? launch_variant<128, true>(*p, tq, tk, tv, a, grid, cs) : launch_variant<128, false>(*p, tq, tk, tv, a, grid, cs);
