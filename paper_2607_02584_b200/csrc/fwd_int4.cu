@@ -7,18 +7,18 @@
 //   warps 16-23   drain: 2 threads per query row (D/2 channels each): online-softmax bookkeeping (m, l, alpha, beta),
 //                 P~V block -> fp32 O registers, epilogue O/l
 //   warp 24       TMEM allocator, then scale loader (Ks[j] * 2^18 log2e/sqrt(D) and Vs[g][:] -> shared rings)
-//   warp 25       TMA producer  : Q tile once, K tiles and V^T tiles (4-stage rings)
-//   warp 26       MMA issuer 2  : P~V (P codes from TMEM x V codes, TMEM)
+//   warp 25       TMA producer  : Q tile once, K tiles (4-stage ring) and V^T tiles (3-stage ring)
+//   warp 26       MMA issuer 2  : P~V (P codes x V codes, both from shared memory, TMEM accumulators)
 //   warp 27       MMA issuer 1  : S = Q K^T (codes x codes, exact, TMEM)
 // With the row-block normaliser (reading 13) the codes of block j depend only on block j, so the two softmax
 // groups work on different blocks concurrently and the running max lives in the drain threads.  Each softmax thread
 // makes two passes over its half row of S in tensor memory in 16-column chunks: pass 1 scales by the key scales, writes
 // t back over S and takes the block row max (exchanged with the partner thread through shared memory); pass 2 reads t:
 // exp2 / row sum / codes.
-// TMEM (512 columns): S[2] at 0/128, two P-code slots of 32 columns at 256, three half-width (D/2 channels) P~V
-// accumulators of 64 columns at 320 used in rotation (half k = 2j+h -> buffer k % 3), so that the P~V MMAs run ahead of
-// the drain instead of alternating with it.  P has its own slots so that an S buffer is released as soon as pass 2 has
-// read it (S(j+2) is issued before P~V(j), hiding the MMA latency).
+// TMEM (512 columns): S[2] at 0/128 and four half-width (D/2 channels) P~V accumulators of 64 columns at 256 (block
+// parity x channel half), so that the P~V MMAs run a block ahead of the drain instead of alternating with it.  The u8 P
+// codes go to four shared-memory tiles (128-byte swizzle, A operand from shared memory), so an S buffer is released as
+// soon as pass 2 has read it (S(j+2) is issued before P~V(j), hiding the MMA latency).
 // The per-block drain is forced by the method: beta (row, block) and Vs (channel, block) change every KV block
 // (PAPER.md:L157 online softmax, L190 per-group V scales), so P~V cannot accumulate across blocks in tensor memory.
 #include <cmath>
@@ -27,18 +27,31 @@
 
 namespace rotattn {
 
+#if defined(ROTATTN_SDONE_RELAXED)
+#define mbar_wait_sdone mbar_wait_relaxed
+#elif defined(ROTATTN_SDONE_SPIN)
+#define mbar_wait_sdone mbar_wait_spin
+#else
+#define mbar_wait_sdone mbar_wait
+#endif
+#if defined(ROTATTN_SEMPTY_SPIN)
+#define mbar_wait_sempty mbar_wait_spin
+#else
+#define mbar_wait_sempty mbar_wait
+#endif
+
 constexpr int kFwdThreads = 896;
 // Warp roles.  Within an SM sub-partition the scheduler favours the highest warp id among the eligible warps, so the
 // latency-critical single-thread roles (MMA issue, TMA) get the highest ids and the throughput roles the lowest.
 constexpr int kWarpScale = 24, kWarpTma = 25, kWarpMmaPV = 26, kWarpMmaS = 27;
 constexpr int K_STAGES = 4;
-constexpr int V_STAGES = 4;
-constexpr int P_SLOTS = 2;
-constexpr int PV_BUFS = 3;       // half-width (D/2 channel) P~V accumulators in rotation
+constexpr int V_STAGES = 3;
+constexpr int P_SLOTS = 4;       // P-code tiles in shared memory (A operand of the P~V MMA)
+constexpr int PV_BUFS = 4;       // half-width (D/2 channel) P~V accumulators in rotation: buffer 2 * (j & 1) + h
 constexpr int AB_RING = 8;
 constexpr int KS_RING = 4;
 constexpr int VS_RING = 4;
-static_assert(K_STAGES == 4 && V_STAGES == 4 && P_SLOTS == 2 && KS_RING == VS_RING, "ring sizes are tied together by the shared completion barriers");
+static_assert(K_STAGES == 4 && P_SLOTS == 4 && PV_BUFS == 4 && V_STAGES <= P_SLOTS && KS_RING == VS_RING, "ring sizes are tied together by the shared completion barriers");
 
 template <int D>
 struct SmemInt4 {
@@ -48,12 +61,14 @@ struct SmemInt4 {
   static constexpr int OFF_Q = 0;
   static constexpr int OFF_K = OFF_Q + Q_BYTES;
   static constexpr int OFF_V = OFF_K + K_STAGES * K_BYTES;
-  static constexpr int OFF_KS = OFF_V + V_STAGES * V_BYTES;           // float [KS_RING][128]
+  static constexpr int P_BYTES = 128 * 128;                           // u8 codes [128 query rows][128 keys], 128-byte swizzle
+  static constexpr int OFF_P = OFF_V + V_STAGES * V_BYTES;
+  static constexpr int OFF_KS = OFF_P + P_SLOTS * P_BYTES;            // float [KS_RING][128]
   static constexpr int OFF_VS = OFF_KS + KS_RING * 128 * 4;           // float [VS_RING][D]
-  static constexpr int OFF_AB = OFF_VS + VS_RING * D * 4;             // float2 [AB_RING][2 halves][128]  (block max, half-row sum)
-  static constexpr int OFF_MX = OFF_AB + AB_RING * 2 * 128 * 8;       // float [2 groups][2 parities][2 halves][128]
+  static constexpr int OFF_AB = OFF_VS + VS_RING * D * 4;             // float [AB_RING][3][128]: block max, half-row sums of the two key halves
+  static constexpr int OFF_MX = OFF_AB + AB_RING * 3 * 128 * 4;       // float [2 groups][2 parities][2 halves][128]
   static constexpr int OFF_BAR = OFF_MX + 2 * 2 * 2 * 128 * 4;        // mbarriers
-  static constexpr int NBAR = 1 + 2 * K_STAGES + 2 * V_STAGES + 2 + P_SLOTS + 2 * PV_BUFS + AB_RING + 2 * KS_RING + 2 * VS_RING;
+  static constexpr int NBAR = 1 + 2 * K_STAGES + V_STAGES + 2 + 2 * P_SLOTS + 2 * PV_BUFS + AB_RING + 2 * KS_RING + 2 * VS_RING;
   static constexpr int OFF_TMEM = OFF_BAR + NBAR * 8;
   static constexpr int TOTAL = OFF_TMEM + 16;
 };
@@ -105,9 +120,10 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   uint8_t* sQ = smem + L::OFF_Q;
   uint8_t* sK = smem + L::OFF_K;
   uint8_t* sV = smem + L::OFF_V;
+  uint8_t* sP = smem + L::OFF_P;
   float* sKs = (float*)(smem + L::OFF_KS);
   float* sVs = (float*)(smem + L::OFF_VS);
-  float2* sAB = (float2*)(smem + L::OFF_AB);
+  float* sAB = (float*)(smem + L::OFF_AB);
   float* sMx = (float*)(smem + L::OFF_MX);
   uint64_t* bars = (uint64_t*)(smem + L::OFF_BAR);
   uint64_t* q_full = bars;
@@ -116,8 +132,8 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   uint64_t* s_done = v_full + V_STAGES;       // [K_STAGES] S(m) complete: -> softmax group m & 1 (S ready), -> TMA (K stage free)
   uint64_t* s_empty = s_done + K_STAGES;      // [2] softmax group -> MMA (count 256): S buffer has been read
   uint64_t* p_full = s_empty + 2;             // [P_SLOTS] softmax group -> MMA (count 256)
-  uint64_t* pv_done = p_full + P_SLOTS;       // [V_STAGES] both halves of P~V(j) complete: -> softmax (P slot free), TMA (V stage free)
-  uint64_t* pvh_done = pv_done + V_STAGES;    // [PV_BUFS] half k = 2j+h of P~V complete -> drain warps of channel half h
+  uint64_t* pv_done = p_full + P_SLOTS;       // [P_SLOTS] both halves of P~V(j) complete: -> softmax (P slot free), TMA (V stage free)
+  uint64_t* pvh_done = pv_done + P_SLOTS;    // [PV_BUFS] half k = 2j+h of P~V complete -> drain warps of channel half h
   uint64_t* pvh_empty = pvh_done + PV_BUFS;   // [PV_BUFS] drain -> MMA (count 128): half buffer is in registers
   uint64_t* ab_full = pvh_empty + PV_BUFS;    // [AB_RING] softmax -> drain (count 256)
   uint64_t* ks_full = ab_full + AB_RING;      // [KS_RING] loader -> softmax (count 32)
@@ -140,7 +156,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     for (int i = 0; i < V_STAGES; ++i) mbar_init(&v_full[i], 1);
     for (int i = 0; i < 2; ++i) mbar_init(&s_empty[i], 256);
     for (int i = 0; i < P_SLOTS; ++i) mbar_init(&p_full[i], 256);
-    for (int i = 0; i < V_STAGES; ++i) mbar_init(&pv_done[i], 1);
+    for (int i = 0; i < P_SLOTS; ++i) mbar_init(&pv_done[i], 1);
     for (int i = 0; i < PV_BUFS; ++i) { mbar_init(&pvh_done[i], 1); mbar_init(&pvh_empty[i], 128); }
     for (int i = 0; i < AB_RING; ++i) mbar_init(&ab_full[i], 256);
     for (int i = 0; i < KS_RING; ++i) { mbar_init(&ks_full[i], 32); mbar_init(&ks_empty[i], 256); }
@@ -152,7 +168,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
-  constexpr uint32_t TM_S = 0, TM_P = 256, TM_PV = 320;     // S[2] x 128 | P[2] x 32 | PV half buffers [3] x 64
+  constexpr uint32_t TM_S = 0, TM_PV = 256;                 // S[2] x 128 | PV half buffers [4] x 64
 
   // register pool of the CTA = 896 x 72; after redistribution 128 x 24 + 512 x 72 + 256 x 96 = 64512 (exactly the pool)
   if (warp >= 24) {
@@ -171,7 +187,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const int m = i, j = i - 2;                                      // K runs two blocks ahead of V
         if (m < nblk) {
           const int s = m % K_STAGES;
-          mbar_wait(&s_done[s], ((m / K_STAGES) & 1) ^ 1);               // S(m-4) has consumed this K stage
+          mbar_wait_relaxed(&s_done[s], ((m / K_STAGES) & 1) ^ 1);               // S(m-4) has consumed this K stage
           if (elect_one()) {
             mbar_arrive_expect_tx(&k_full[s], L::K_BYTES);
             tma_load_3d(sK + s * L::K_BYTES, &tmK, &k_full[s], 0, m * kTile, bh);
@@ -180,7 +196,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         }
         if (j >= 0) {
           const int s = j % V_STAGES;
-          mbar_wait(&pv_done[s], ((j / V_STAGES) & 1) ^ 1);              // P~V(j-4) has consumed this V stage
+          if (j >= V_STAGES) mbar_wait_relaxed(&pv_done[(j - V_STAGES) % P_SLOTS], ((j - V_STAGES) / P_SLOTS) & 1);   // P~V(j-3) has consumed this V stage
           if (elect_one()) {
             mbar_arrive_expect_tx(&v_full[s], L::V_BYTES);
             tma_load_3d(sV + s * L::V_BYTES, &tmV, &v_full[s], j * kTile, 0, bh);
@@ -197,9 +213,9 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       for (int m = 0; m < nblk; ++m) {
         const int st = m % K_STAGES, b = m & 1;
         ROTATTN_STAMP(m, 4);
-        mbar_wait(&k_full[st], (m / K_STAGES) & 1);
+        mbar_wait_relaxed(&k_full[st], (m / K_STAGES) & 1);
         ROTATTN_STAMP(m, 5);
-        if (m >= 2) mbar_wait(&s_empty[b], ((m >> 1) - 1) & 1);          // softmax has read S(m-2) out of this buffer
+        if (m >= 2) mbar_wait_sempty(&s_empty[b], ((m >> 1) - 1) & 1);          // softmax has read S(m-2) out of this buffer
         tc_fence_after();
         ROTATTN_STAMP(m, 6);
         if (elect_one()) {
@@ -215,28 +231,28 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     } else if (warp == kWarpMmaPV) {
       // ---------------------------------------------------------------- MMA issuer 2: PV = P~(j) V(j)
       constexpr uint32_t idesc_pv = umma_idesc(1, 0, 0, 128, D / 2);
-      int buf = 0; uint32_t bpar = 1;                                    // rotation state of half k = 2j + h: k % 3, ((k / 3) & 1) ^ 1
       for (int j = 0; j < nblk; ++j) {
         const int slot = j % P_SLOTS, vst = j % V_STAGES;
-        mbar_wait(&v_full[vst], (j / V_STAGES) & 1);
-        mbar_wait(&p_full[slot], (j / P_SLOTS) & 1);
+        mbar_wait_relaxed(&v_full[vst], (j / V_STAGES) & 1);
+        mbar_wait_relaxed(&p_full[slot], (j / P_SLOTS) & 1);
         ROTATTN_STAMP(j, 1);
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
-          mbar_wait(&pvh_empty[buf], bpar);                              // drain has read half k-3 out of this buffer
+          const int buf = 2 * (j & 1) + h;
+          mbar_wait_relaxed(&pvh_empty[buf], ((j >> 1) & 1) ^ 1);                // drain has read half (j-2, h) out of this buffer
           tc_fence_after();
           if (h == 0) ROTATTN_STAMP(j, 3);
           if (elect_one()) {
             // V^T tile: channel half h starts D/2 rows (= D/2 * 128 B, whole 1024-byte swizzle atoms) into the tile
+            const uint64_t pd = umma_desc_k128(smem_u32(sP + slot * L::P_BYTES));
             const uint64_t vd = umma_desc_k128(smem_u32(sV + vst * L::V_BYTES + h * (D / 2) * 128));
 #pragma unroll
             for (int k = 0; k < 4; ++k)
-              mma_ts<MmaKind::F8F6F4>(tmem_base + TM_PV + buf * 64, tmem_base + TM_P + slot * 32 + 8 * k, vd + 2 * k, idesc_pv, k != 0);
+              mma_ss<MmaKind::F8F6F4>(tmem_base + TM_PV + buf * 64, pd + 2 * k, vd + 2 * k, idesc_pv, k != 0);
             tc_commit(&pvh_done[buf]);                                   // -> drain warps of this channel half
-            if (h == 1) tc_commit(&pv_done[vst]);                        // -> softmax (P slot free), TMA (V stage free)
+            if (h == 1) tc_commit(&pv_done[slot]);                        // -> softmax (P slot free), TMA (V stage free)
           }
           __syncwarp();
-          if (++buf == PV_BUFS) { buf = 0; bpar ^= 1; }
         }
         ROTATTN_STAMP(j, 9);
       }
@@ -254,11 +270,11 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         }
 #pragma unroll
         for (int i = 0; i < D / 32; ++i) vv[i] = vsrc[(size_t)j * D + i * 32 + lane];
-        mbar_wait(&ks_empty[s], ((j / KS_RING) & 1) ^ 1);
+        mbar_wait_relaxed(&ks_empty[s], ((j / KS_RING) & 1) ^ 1);
 #pragma unroll
         for (int i = 0; i < 4; ++i) sKs[s * 128 + i * 32 + lane] = kv[i];
         mbar_arrive(&ks_full[s]);
-        mbar_wait(&vs_empty[s], ((j / VS_RING) & 1) ^ 1);
+        mbar_wait_relaxed(&vs_empty[s], ((j / VS_RING) & 1) ^ 1);
 #pragma unroll
         for (int i = 0; i < D / 32; ++i) sVs[s * D + i * 32 + lane] = vv[i];
         mbar_arrive(&vs_full[s]);
@@ -285,7 +301,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       const int nvalid = min(kTile, a.N - j * kTile) - cb;   // valid keys of this half; < 64 only on the ragged last block
       const bool ragged = nvalid < 64;
       mbar_wait(&ks_full[ring], (j / KS_RING) & 1);
-      mbar_wait(&s_done[j % K_STAGES], (j / K_STAGES) & 1);
+      mbar_wait_sdone(&s_done[j % K_STAGES], (j / K_STAGES) & 1);
       tc_fence_after();
       ROTATTN_STAMP(j, 0);
       uint32_t va[16], vb[16], tt[16];
@@ -303,7 +319,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           for (int i = 0; i < 16; ++i)
             a.S_dump[(size_t)r * a.npad + j * kTile + cb + c * 16 + i] = (int32_t)(__uint_as_float(cur[i]) * kAccScale);
         }
-#if defined(ROTATTN_ABL) && ROTATTN_ABL == 3      // development ablation: no pass-1 arithmetic / write-back
+#if defined(ROTATTN_ABL) && (ROTATTN_ABL == 3 || ROTATTN_ABL == 6)      // development ablation: no pass-1 arithmetic / write-back
         mx0 = fmaxf(mx0, __uint_as_float(cur[0]));
 #else
         if (ragged) chunk_scale_max<true>(cur, ks2 + c * 8, nvalid - c * 16, tt, mx0, mx1);
@@ -323,11 +339,11 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       const float mt = qs * tmax;                        // block row max of s * log2e
       const float nref = LOG2_LEVELS - mt;
       const float2 nref2 = make_float2(nref, nref);
-      if (j >= P_SLOTS) mbar_wait(&pv_done[(j - P_SLOTS) % V_STAGES], ((j - P_SLOTS) / V_STAGES) & 1);   // P~V(j-2) has consumed this P slot
+      mbar_wait(&pv_done[slot], ((j / P_SLOTS) & 1) ^ 1);            // P~V(j-4) has consumed this P slot
       ROTATTN_STAMP(j, 2);
       // ---- pass 2: LEVELS * P^, row sum, codes -> u8 P tile slot
       float2 ls0 = make_float2(0.f, 0.f), ls1 = make_float2(0.f, 0.f);
-      const uint32_t p_addr = tmem_base + lane_off + TM_P + slot * 32 + 16 * h;
+      uint8_t* p_row = sP + slot * L::P_BYTES + r * 128;             // 16-byte chunk q of row r lives at chunk q ^ (r & 7)
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
         tmem_wait_ld();
@@ -336,17 +352,21 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         if (c < 3) tmem_ld16(s_addr + (c + 1) * 16, nxt);
         else { tc_fence_before(); mbar_arrive(&s_empty[g]); }          // this thread is done with the S buffer
         uint32_t pw[4];
+#if defined(ROTATTN_ABL) && (ROTATTN_ABL == 4 || ROTATTN_ABL == 6)   // development ablation: no pass-2 arithmetic
+        pw[0] = cur[0]; pw[1] = cur[1]; pw[2] = cur[2]; pw[3] = cur[3];
+#else
         chunk_exp(cur, qs2, nref2, ls0, ls1, pw);
+#endif
         if (DEBUG) {
 #pragma unroll
           for (int q = 0; q < 4; ++q) *reinterpret_cast<uint32_t*>(a.P_dump + (size_t)r * a.npad + j * kTile + cb + c * 16 + q * 4) = pw[q];
         }
-        tmem_st4(p_addr + c * 4, pw);
+        *reinterpret_cast<uint4*>(p_row + (((4 * h + c) ^ (r & 7)) << 4)) = make_uint4(pw[0], pw[1], pw[2], pw[3]);
       }
-      sAB[(abslot * 2 + h) * 128 + r] = make_float2(mt, (ls0.x + ls0.y) + (ls1.x + ls1.y));
+      if (h == 0) sAB[(abslot * 3) * 128 + r] = mt;
+      sAB[(abslot * 3 + 1 + h) * 128 + r] = (ls0.x + ls0.y) + (ls1.x + ls1.y);
       ROTATTN_STAMP(j, 3);
-      tmem_wait_st();
-      tc_fence_before();
+      fence_proxy_async_smem();                          // P codes (generic-proxy stores) -> visible to the MMA (async proxy)
       mbar_arrive(&p_full[slot]);
       ROTATTN_STAMP(j, 4);
       mbar_arrive(&ab_full[abslot]);
@@ -361,66 +381,60 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     float2 o2[DH / 2];
 #pragma unroll
     for (int d = 0; d < DH / 2; ++d) o2[d] = make_float2(0.f, 0.f);
-    float m_run = -INFINITY, l_run = 0.f;
-    int buf = h; uint32_t bpar = 0;                  // rotation state of half k = 2j + h: k % 3, (k / 3) & 1
+    // Online softmax bookkeeping (L157) with a lazily updated reference max: O and l are kept relative to m_ref, which
+    // only moves when a block max exceeds it by more than 2^8 (fp32 has the headroom), so the common path is
+    // O += beta * pv * Vs with beta = exp2(mt - m_ref) and no rescale of the 64 accumulators.
+    constexpr float kLazy = 8.f;
+    float m_ref = -INFINITY, l_run = 0.f;
     for (int j = 0; j < nblk; ++j) {
-      // online softmax bookkeeping (L157): m' = max(m, mt); alpha = exp(m - m'); beta = exp(mt - m'); l = alpha l + beta sum(P^)
       const int abslot = j % AB_RING;
       ROTATTN_STAMP(j, 0);
-      mbar_wait(&ab_full[abslot], (j / AB_RING) & 1);
+      mbar_wait_relaxed(&ab_full[abslot], (j / AB_RING) & 1);
       ROTATTN_STAMP(j, 1);
-      const float2 ms0 = sAB[(abslot * 2 + 0) * 128 + r], ms1 = sAB[(abslot * 2 + 1) * 128 + r];
-      const float m_new = fmaxf(m_run, ms0.x);
-      const float alpha = ex2_approx(m_run - m_new);                   // first block: exp2(-inf) = 0
-      const float beta = ex2_approx(ms0.x - m_new);
-      l_run = alpha * l_run + beta * (ms0.y + ms1.y);                  // in units of LEVELS (cancels in O/l)
-      m_run = m_new;
-      const float cf = beta * kAccScale;                               // undoes the 2^-18 of the E4M3 code products
-      const float2 c2 = make_float2(cf, cf), a2 = make_float2(alpha, alpha);
-      const bool keep = __all_sync(0xffffffffu, alpha == 1.f);         // no new row max in this warp's 32 rows
+      const float mt = sAB[(abslot * 3) * 128 + r];
+      const float bsum = sAB[(abslot * 3 + 1) * 128 + r] + sAB[(abslot * 3 + 2) * 128 + r];
       const int vring = j % VS_RING;
-      mbar_wait(&vs_full[vring], (j / VS_RING) & 1);
-      const float2* vsb2 = reinterpret_cast<const float2*>(sVs + vring * D + h * DH);
-      mbar_wait(&pvh_done[buf], bpar);
+      const int buf = 2 * (j & 1) + h;
+      const uint32_t pv_addr = tmem_base + lane_off + TM_PV + buf * 64;
+      mbar_wait_relaxed(&vs_full[vring], (j / VS_RING) & 1);
+      mbar_wait_relaxed(&pvh_done[buf], (j >> 1) & 1);
       tc_fence_after();
       ROTATTN_STAMP(j, 2);
+      uint32_t va[16], vb[16];
+      tmem_ld16(pv_addr, va);                                          // in flight across the bookkeeping below
+      if (__any_sync(0xffffffffu, mt > m_ref + kLazy)) {               // rare after the first blocks (warp-uniform branch)
+        const float m_new = (mt > m_ref + kLazy) ? mt : m_ref;
+        const float alpha = ex2_approx(m_ref - m_new);                 // first block: exp2(-inf) = 0; unchanged rows: 1
+        const float2 a2 = make_float2(alpha, alpha);
+#pragma unroll
+        for (int d = 0; d < DH / 2; ++d) o2[d] = fmul2(o2[d], a2);
+        l_run *= alpha;
+        m_ref = m_new;
+      }
+      const float beta = ex2_approx(mt - m_ref);                       // <= 2^8
+      l_run = fmaf(beta, bsum, l_run);                                 // in units of LEVELS (cancels in O/l)
+      const float cf = beta * kAccScale;                               // undoes the 2^-18 of the E4M3 code products
+      const float2 c2 = make_float2(cf, cf);
+      const float2* vsb2 = reinterpret_cast<const float2*>(sVs + vring * D + h * DH);
 #pragma unroll
       for (int cc = 0; cc < DH / 16; ++cc) {
-        uint32_t v[16];
-        tmem_ld16(tmem_base + lane_off + TM_PV + buf * 64 + cc * 16, v);
         tmem_wait_ld();
+        uint32_t(&cur)[16] = (cc & 1) ? vb : va;
+        uint32_t(&nxt)[16] = (cc & 1) ? va : vb;
         ROTATTN_STAMP(j, 4 + cc);
-        if (cc == DH / 16 - 1) {                                       // PV buffer is in registers now
-          tc_fence_before();
-          mbar_arrive(&pvh_empty[buf]);
-        }
-#if defined(ROTATTN_ABL) && ROTATTN_ABL == 2      // development ablation: no drain arithmetic
-        o2[cc].x += __uint_as_float(v[0]);
-        if (false) {
-#else
-        if (keep) {
-#endif
+        if (cc + 1 < DH / 16) tmem_ld16(pv_addr + (cc + 1) * 16, nxt);
+        else { tc_fence_before(); mbar_arrive(&pvh_empty[buf]); }      // this half-width accumulator is in registers now
+#if !(defined(ROTATTN_ABL) && (ROTATTN_ABL == 2 || ROTATTN_ABL == 6))
 #pragma unroll
-          for (int d = 0; d < 8; ++d) {
-            const float2 y = fmul2(make_float2(__uint_as_float(v[2 * d]), __uint_as_float(v[2 * d + 1])), vsb2[cc * 8 + d]);
-            o2[cc * 8 + d] = ffma2(y, c2, o2[cc * 8 + d]);             // O += beta * pv * Vs[g][d]
-          }
+        for (int d = 0; d < 8; ++d) {
+          const float2 y = fmul2(make_float2(__uint_as_float(cur[2 * d]), __uint_as_float(cur[2 * d + 1])), vsb2[cc * 8 + d]);
+          o2[cc * 8 + d] = ffma2(y, c2, o2[cc * 8 + d]);               // O += beta * pv * Vs[g][d]
         }
-#if defined(ROTATTN_ABL) && ROTATTN_ABL == 2
-        else if (false) {
 #else
-        else {
+        o2[cc].x += __uint_as_float(cur[0]);
 #endif
-#pragma unroll
-          for (int d = 0; d < 8; ++d) {
-            const float2 y = fmul2(make_float2(__uint_as_float(v[2 * d]), __uint_as_float(v[2 * d + 1])), vsb2[cc * 8 + d]);
-            o2[cc * 8 + d] = ffma2(o2[cc * 8 + d], a2, fmul2(y, c2));  // O = alpha O + beta * pv * Vs[g][d]
-          }
-        }
       }
       mbar_arrive(&vs_empty[vring]);
-      buf += 2;                                       // k -> k + 2
-      if (buf >= PV_BUFS) { buf -= PV_BUFS; bpar ^= 1; }
       ROTATTN_STAMP(j, 3);
     }
     const float inv_l = 1.f / l_run;

@@ -27,6 +27,15 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
 }
 __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
   uint32_t ok;
+#ifdef ROTATTN_WAIT_HINT_NS
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok)
+      : "r"(smem_u32(bar)), "r"(parity), "r"((uint32_t)ROTATTN_WAIT_HINT_NS)
+      : "memory");
+#else
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
       "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
@@ -34,16 +43,48 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
       : "=r"(ok)
       : "r"(smem_u32(bar)), "r"(parity)
       : "memory");
+#endif
   return ok != 0;
 }
 // Bounded wait: a protocol bug must not hang the GPU box (a hang there is a strike).  try_wait suspends the thread in
-// hardware for a bounded time per call, so the retry loop is cold; after 2^26 retries (seconds) the thread traps,
-// which surfaces as a CUDA error at the next API call.
+// hardware for a bounded time per call; after 2^26 retries (seconds) the thread traps, which surfaces as a CUDA error
+// at the next API call.  mbar_wait spins (latency-critical hand-offs); mbar_wait_relaxed backs off between retries so
+// that a waiting warp does not take issue slots from the working warps of its SM sub-partition.
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   if (mbar_try_wait(bar, parity)) return;
   uint32_t spins = 0;
 #pragma unroll 1
   while (!mbar_try_wait(bar, parity)) {
+    if (++spins > (1u << 26)) __trap();
+  }
+}
+// Non-suspending poll (mbarrier.test_wait): lowest wake-up latency, for the hand-offs on the critical cycle.
+__device__ __forceinline__ bool mbar_test_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok)
+      : "r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait_spin(uint64_t* bar, uint32_t parity) {
+  uint32_t spins = 0;
+#pragma unroll 1
+  while (!mbar_test_wait(bar, parity)) {
+    if (++spins > (1u << 28)) __trap();
+  }
+}
+__device__ __forceinline__ void mbar_wait_relaxed(uint64_t* bar, uint32_t parity) {
+  if (mbar_try_wait(bar, parity)) return;
+  uint32_t spins = 0;
+#pragma unroll 1
+  while (!mbar_try_wait(bar, parity)) {
+#ifdef ROTATTN_BACKOFF_NS
+    __nanosleep(ROTATTN_BACKOFF_NS);
+#endif
     if (++spins > (1u << 26)) __trap();
   }
 }
