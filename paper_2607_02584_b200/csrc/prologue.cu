@@ -29,12 +29,15 @@ __device__ __forceinline__ int quant_code(float y, float inv) {
 // so tcgen05 kind::f8f6f4 multiplies and accumulates the integer codes exactly, scaled by 2^-18, in fp32.
 __device__ __forceinline__ uint32_t code_byte(int c) { return (uint32_t)(abs(c) | ((c >> 24) & 0x80)); }
 
+constexpr int kPrepTok = 4;       // tokens per warp iteration: all their loads are issued before any arithmetic (bytes in flight)
+
 template <int D, int ROT>
-__global__ void __launch_bounds__(256) prepare_qk_kernel(const PrepArgs a) {
+__global__ void __launch_bounds__(256, 2) prepare_qk_kernel(const PrepArgs a) {
   constexpr int CPL = D / 32;       // channels per lane
   constexpr int PPL = CPL / 2;      // RoPE pairs per lane
   constexpr int WPB = 8;            // warps per block
-  __shared__ float ybuf[WPB][2][D]; // HALF-rotation exchange buffer
+  constexpr int TOK = kPrepTok;
+  __shared__ float ybuf[ROT == ROTATTN_ROT_HALF ? WPB : 1][TOK][2][D];   // HALF-rotation exchange buffer
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
   // ---- per-lane constants ----
@@ -65,91 +68,157 @@ __global__ void __launch_bounds__(256) prepare_qk_kernel(const PrepArgs a) {
       partner[j] = role_u[j] ? c + P : c - P;
       float4 r = a.rot ? a.rot[blk] : make_float4(0.70710678118654752440f, 0.70710678118654752440f,
                                                   0.70710678118654752440f, -0.70710678118654752440f);
-      ca[j] = role_u[j] ? r.x : r.y;   // multiplies u
-      cb[j] = role_u[j] ? r.z : r.w;   // multiplies v
+      // u' = u r00 + v r10 (this lane holds u), v' = u r01 + v r11 (this lane holds v): own value times ca + partner times cb
+      ca[j] = role_u[j] ? r.x : r.w;
+      cb[j] = role_u[j] ? r.z : r.y;
     }
   }
 
-  const long long wstride = (long long)gridDim.x * WPB;
-  for (long long tok = (long long)blockIdx.x * WPB + warp; tok < a.total; tok += wstride) {
-    const int n = (int)(tok % a.N);
-    int pos[3];
-    if (n < a.n_rope) {
-      pos[2] = n % a.gw; int r = n / a.gw; pos[1] = r % a.gh; pos[0] = r / a.gh;
-    } else {
-      pos[0] = a.gt; pos[1] = a.gh; pos[2] = a.gw;     // no-RoPE rows
-    }
-    float4 A[PPL];
+  // blockIdx.y = (b,h); the warps of the grid's x dimension stride over that head's tokens, TOK consecutive ones at a time
+  const long long head0 = (long long)blockIdx.y * a.N;
+  const int nstride = gridDim.x * WPB * TOK;
+  for (int n0 = (blockIdx.x * WPB + warp) * TOK; n0 < a.N; n0 += nstride) {
+    // (t,h,w) of the first token by two 32-bit divisions; the following ones by carry propagation
+    int pw = n0 % a.gw, pr = n0 / a.gw;
+    int ph = pr % a.gh, pt = pr / a.gh;
+    // ---- load phase: TOK tokens x (Q, K) + their coefficient rows, all independent
+    float4 A[TOK][PPL];
+    __half hx[TOK][2][CPL];
 #pragma unroll
-    for (int i = 0; i < PPL; ++i) A[i] = __ldg(a.coef + cbase[i] + pos[caxis[i]] * cstride[i]);
-
-    float y[2][CPL];
+    for (int t = 0; t < TOK; ++t) {
+      const int n = n0 + t;
+      if (n < a.N) {
+        const long long tok = head0 + n;
 #pragma unroll
-    for (int m = 0; m < 2; ++m) {
-      const __half* src = a.X[m] + tok * D + lane * CPL;
-      __half hx[CPL];
-      if (CPL == 4) { uint2 v = *reinterpret_cast<const uint2*>(src); *reinterpret_cast<uint2*>(hx) = v; }
-      else { uint32_t v = *reinterpret_cast<const uint32_t*>(src); *reinterpret_cast<uint32_t*>(hx) = v; }
+        for (int m = 0; m < 2; ++m) {
+          const __half* src = a.X[m] + tok * D + lane * CPL;
+          if (CPL == 4) *reinterpret_cast<uint2*>(hx[t][m]) = __ldcs(reinterpret_cast<const uint2*>(src));
+          else *reinterpret_cast<uint32_t*>(hx[t][m]) = __ldcs(reinterpret_cast<const uint32_t*>(src));
+        }
+        int pos[3];
+        if (n < a.n_rope) {
+          pos[0] = pt; pos[1] = ph; pos[2] = pw;
+        } else {
+          pos[0] = a.gt; pos[1] = a.gh; pos[2] = a.gw;     // no-RoPE rows
+        }
 #pragma unroll
-      for (int i = 0; i < PPL; ++i) {
-        float x0 = __half2float(hx[2 * i]), x1 = __half2float(hx[2 * i + 1]);
-        y[m][2 * i]     = __fadd_rn(__fmul_rn(x0, A[i].x), __fmul_rn(x1, A[i].z));
-        y[m][2 * i + 1] = __fadd_rn(__fmul_rn(x0, A[i].y), __fmul_rn(x1, A[i].w));
+        for (int i = 0; i < PPL; ++i) A[t][i] = __ldg(a.coef + cbase[i] + pos[caxis[i]] * cstride[i]);
       }
+      if (++pw == a.gw) { pw = 0; if (++ph == a.gh) { ph = 0; ++pt; } }
     }
+    // ---- RoPE (merged with the interleaved rotation through the table)
+    float y[TOK][2][CPL];
+#pragma unroll
+    for (int t = 0; t < TOK; ++t)
+#pragma unroll
+      for (int m = 0; m < 2; ++m)
+#pragma unroll
+        for (int i = 0; i < PPL; ++i) {
+          float x0 = __half2float(hx[t][m][2 * i]), x1 = __half2float(hx[t][m][2 * i + 1]);
+          y[t][m][2 * i]     = __fadd_rn(__fmul_rn(x0, A[t][i].x), __fmul_rn(x1, A[t][i].z));
+          y[t][m][2 * i + 1] = __fadd_rn(__fmul_rn(x0, A[t][i].y), __fmul_rn(x1, A[t][i].w));
+        }
     if (ROT == ROTATTN_ROT_HALF) {
 #pragma unroll
-      for (int m = 0; m < 2; ++m)
+      for (int t = 0; t < TOK; ++t)
 #pragma unroll
-        for (int j = 0; j < CPL; ++j) ybuf[warp][m][lane * CPL + j] = y[m][j];
+        for (int m = 0; m < 2; ++m) {
+          if (CPL == 4) *reinterpret_cast<float4*>(&ybuf[warp][t][m][lane * CPL]) = make_float4(y[t][m][0], y[t][m][1], y[t][m][2], y[t][m][3]);
+          else *reinterpret_cast<float2*>(&ybuf[warp][t][m][lane * CPL]) = make_float2(y[t][m][0], y[t][m][1]);
+        }
       __syncwarp();
 #pragma unroll
-      for (int m = 0; m < 2; ++m)
+      for (int t = 0; t < TOK; ++t)
 #pragma unroll
-        for (int j = 0; j < CPL; ++j) {
-          float other = ybuf[warp][m][partner[j]];
-          float u = role_u[j] ? y[m][j] : other;
-          float v = role_u[j] ? other : y[m][j];
-          y[m][j] = __fadd_rn(__fmul_rn(u, ca[j]), __fmul_rn(v, cb[j]));
-        }
+        for (int m = 0; m < 2; ++m)
+#pragma unroll
+          for (int j = 0; j < CPL; ++j) {
+            const float other = ybuf[warp][t][m][partner[j]];
+            y[t][m][j] = __fadd_rn(__fmul_rn(y[t][m][j], ca[j]), __fmul_rn(other, cb[j]));   // fp32 addition commutes exactly
+          }
       __syncwarp();
     }
+    // ---- per-token amax (all TOK x 2 reductions interleaved), quantise, store
+    float amax[TOK][2];
 #pragma unroll
-    for (int m = 0; m < 2; ++m) {
-      float amax = 0.f;
+    for (int t = 0; t < TOK; ++t)
 #pragma unroll
-      for (int j = 0; j < CPL; ++j) amax = fmaxf(amax, fabsf(y[m][j]));
+      for (int m = 0; m < 2; ++m) {
+        float v = 0.f;
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
-      const float scale = __fdiv_rn(amax, 7.0f);
-      const float inv = amax > 0.f ? __fdiv_rn(7.0f, amax) : 0.f;
-      int c[CPL];
-#pragma unroll
-      for (int j = 0; j < CPL; ++j) c[j] = quant_code(y[m][j], inv);
-      if (CPL == 4) {
-        uint16_t pk = (uint16_t)((c[0] & 0xF) | ((c[1] & 0xF) << 4) | ((c[2] & 0xF) << 8) | ((c[3] & 0xF) << 12));
-        *reinterpret_cast<uint16_t*>(a.X4[m] + tok * (D / 2) + lane * 2) = pk;
-      } else {
-        a.X4[m][tok * (D / 2) + lane] = (uint8_t)((c[0] & 0xF) | ((c[1] & 0xF) << 4));
+        for (int j = 0; j < CPL; ++j) v = fmaxf(v, fabsf(y[t][m][j]));
+        amax[t][m] = v;
       }
-      if (lane == 0) a.Xs[m][tok] = scale;
-      if (a.X8[m]) {
-        int8_t* dst = a.X8[m] + tok * kQKRowBytes;
-        if (CPL == 4) {
-          uint32_t w = code_byte(c[0]) | (code_byte(c[1]) << 8) | (code_byte(c[2]) << 16) | (code_byte(c[3]) << 24);
-          *reinterpret_cast<uint32_t*>(dst + lane * 4) = w;
-        } else {
-          *reinterpret_cast<uint16_t*>(dst + lane * 2) = (uint16_t)(code_byte(c[0]) | (code_byte(c[1]) << 8));
-          *reinterpret_cast<uint16_t*>(dst + 64 + lane * 2) = 0;      // zero pad to a 128-byte row
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+      for (int t = 0; t < TOK; ++t)
+#pragma unroll
+        for (int m = 0; m < 2; ++m) amax[t][m] = fmaxf(amax[t][m], __shfl_xor_sync(0xffffffffu, amax[t][m], o));
+    // scale = amax / 7 and inv = 7 / amax are IEEE divisions: lane (2 t + m) computes the pair once, then broadcast
+    float my_scale = 0.f, my_inv = 0.f;
+    {
+      float am = 0.f;
+#pragma unroll
+      for (int t = 0; t < TOK; ++t)
+#pragma unroll
+        for (int m = 0; m < 2; ++m) am = (lane == 2 * t + m) ? amax[t][m] : am;
+      if (lane < 2 * TOK) {
+        my_scale = __fdiv_rn(am, 7.0f);
+        my_inv = am > 0.f ? __fdiv_rn(7.0f, am) : 0.f;
+      }
+    }
+#pragma unroll
+    for (int t = 0; t < TOK; ++t) {
+      if (n0 + t >= a.N) break;
+      const long long tok = head0 + n0 + t;
+#pragma unroll
+      for (int m = 0; m < 2; ++m) {
+        const float scale = __shfl_sync(0xffffffffu, my_scale, 2 * t + m);
+        const float inv = __shfl_sync(0xffffffffu, my_inv, 2 * t + m);
+        // code = rne(y * inv) is in [-7,7] without clamping (|y| <= amax and inv = rn(7/amax) give |y*inv| < 7.5).
+        // fs = q + 1.5*2^23 holds the two's-complement code in its low byte, fa = |q| + 1.5*2^23 the magnitude.
+        uint32_t fs[CPL], fa[CPL], yb[CPL];
+#pragma unroll
+        for (int j = 0; j < CPL; ++j) {
+          const float q = __fmul_rn(y[t][m][j], inv);
+          fs[j] = __float_as_uint(__fadd_rn(q, 12582912.f));
+          fa[j] = __float_as_uint(__fadd_rn(fabsf(q), 12582912.f));
+          yb[j] = __float_as_uint(q);
         }
-      }
-      if (a.X16[m]) {
-        __half* dst = a.X16[m] + tok * D + lane * CPL;
-        __half hy[CPL];
+        if (CPL == 4) {
+          const uint32_t n01 = (fs[0] & 0xFu) | ((fs[1] << 4) & 0xF0u), n23 = (fs[2] & 0xFu) | ((fs[3] << 4) & 0xF0u);
+          *reinterpret_cast<uint16_t*>(a.X4[m] + tok * (D / 2) + lane * 2) = (uint16_t)__byte_perm(n01, n23, 0x0040);
+        } else {
+          a.X4[m][tok * (D / 2) + lane] = (uint8_t)((fs[0] & 0xFu) | ((fs[1] << 4) & 0xF0u));
+        }
+        if (lane == 0) a.Xs[m][tok] = scale;
+        if (a.X8[m]) {
+          // sign-magnitude operand bytes (code_byte): magnitude bytes | sign bits of q (a zero code has q = +-0 or |q| < 0.5:
+          // its sign must not be stored, hence the mask with the non-zero test folded into the magnitude: -0 byte is avoided
+          // by taking the sign only where the magnitude byte is non-zero)
+          int8_t* dst = a.X8[m] + tok * kQKRowBytes;
+          if (CPL == 4) {
+            const uint32_t mag = __byte_perm(__byte_perm(fa[0], fa[1], 0x0040), __byte_perm(fa[2], fa[3], 0x0040), 0x5410);
+            const uint32_t sgn = __byte_perm(__byte_perm(yb[0], yb[1], 0x0073), __byte_perm(yb[2], yb[3], 0x0073), 0x5410);
+            const uint32_t nz = ((mag + 0x7F7F7F7Fu) & 0x80808080u);     // 0x80 in every byte whose magnitude is non-zero
+            *reinterpret_cast<uint32_t*>(dst + lane * 4) = mag | (sgn & nz);
+          } else {
+            const uint32_t mag = __byte_perm(fa[0], fa[1], 0x0040) & 0xFFFFu;
+            const uint32_t sgn = __byte_perm(yb[0], yb[1], 0x0073) & 0xFFFFu;
+            const uint32_t nz = ((mag + 0x7F7Fu) & 0x8080u);
+            *reinterpret_cast<uint16_t*>(dst + lane * 2) = (uint16_t)(mag | (sgn & nz));
+            *reinterpret_cast<uint16_t*>(dst + 64 + lane * 2) = 0;      // zero pad to a 128-byte row
+          }
+        }
+        if (a.X16[m]) {
+          __half* dst = a.X16[m] + tok * D + lane * CPL;
+          __half hy[CPL];
 #pragma unroll
-        for (int j = 0; j < CPL; ++j) hy[j] = __float2half_rn(y[m][j]);
-        if (CPL == 4) *reinterpret_cast<uint2*>(dst) = *reinterpret_cast<uint2*>(hy);
-        else *reinterpret_cast<uint32_t*>(dst) = *reinterpret_cast<uint32_t*>(hy);
+          for (int j = 0; j < CPL; ++j) hy[j] = __float2half_rn(y[t][m][j]);
+          if (CPL == 4) *reinterpret_cast<uint2*>(dst) = *reinterpret_cast<uint2*>(hy);
+          else *reinterpret_cast<uint32_t*>(dst) = *reinterpret_cast<uint32_t*>(hy);
+        }
       }
     }
   }
@@ -161,7 +230,7 @@ __global__ void __launch_bounds__(256) prepare_qk_kernel(const PrepArgs a) {
 // through a swizzled shared tile, as int8 [D, npad] (K-major B operand of the P~V MMA).
 // ------------------------------------------------------------------------------------------------
 template <int D>
-__global__ void __launch_bounds__(256) quant_v_kernel(const __half* __restrict__ V, uint8_t* __restrict__ V4,
+__global__ void __launch_bounds__(256, 3) quant_v_kernel(const __half* __restrict__ V, uint8_t* __restrict__ V4,
                                                       float* __restrict__ Vs, int8_t* __restrict__ V8T,
                                                       int N, int nG, int npad) {
   constexpr int CR = D / 8;           // 16-byte chunks per row
@@ -306,10 +375,11 @@ static int launch_prepare(const rotattn_params& p, const PrepArgs& a, cudaStream
   int dev = 0, sms = 148;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  long long blocks_needed = (a.total + 7) / 8;
-  long long cap = (long long)sms * 8 * 4;          // 8 CTAs of 8 warps per SM, 4 tokens per warp minimum
-  unsigned grid = (unsigned)(blocks_needed < cap ? blocks_needed : cap);
-  if (grid == 0) grid = 1;
+  const int BH = p.B * p.H;
+  long long blocks_needed = ((long long)a.N + 8 * kPrepTok - 1) / (8 * kPrepTok);     // per (b,h)
+  long long cap = ((long long)sms * 2 * 8 + BH - 1) / BH;                             // 2 resident CTAs per SM, 8 waves at most
+  dim3 grid((unsigned)(blocks_needed < cap ? blocks_needed : cap), (unsigned)BH);
+  if (grid.x == 0) grid.x = 1;
   switch (p.rot_mode) {
     case ROTATTN_ROT_NONE:
     case ROTATTN_ROT_INTERLEAVED:   // merged into the table: same kernel as plain RoPE
