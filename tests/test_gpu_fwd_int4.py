@@ -151,3 +151,60 @@ def test_full_size_wan13b_row_sample():
         qc, qs, kc, ks, vc, vs = _oracle_inputs(res, 0, h)
         Ow = orc.o_quant(po, qc, qs, kc, ks, vc, vs, rows=rows)
         _check_o(res['O'][0, h].float().cpu().numpy()[rows], Ow)
+
+
+def _full_size_case(w, heads, p_mode=orc.P_ASYM15, rot_mode=orc.ROT_HALF, n_tiles=3):
+    """Full N and D of a BASELINE.json config on a seeded subset of its heads (heads are independent units):
+    prologue codes bit-exact on the sampled rows' inputs, S/P dumps on the ragged last tile, O on a seeded row sample."""
+    api = _api()
+    q, k, v = syn.gen_all(w, heads=heads)
+    res = api.run_int4(w, q, k, v, rot_mode=rot_mode, p_mode=p_mode)
+    torch.cuda.synchronize()
+    po = orc.Params(w.B, len(heads), w.N, w.D, w.grid, w.pairs, rot_mode=rot_mode, p_mode=p_mode)
+    for i, h in enumerate(heads):
+        rows = syn.sample_rows(w, n_tiles=n_tiles, head=h)
+        tiles = sorted(set((rows // 128).tolist()))
+        _check_tile(api, res, po, 0, i, tiles[-1], p_mode, orc.NORM_ROWBLOCK)
+        qc, qs, kc, ks, vc, vs = _oracle_inputs(res, 0, i)
+        Ow = orc.o_quant(po, qc, qs, kc, ks, vc, vs, rows=rows, p_mode=p_mode)
+        _check_o(res['O'][0, i].float().cpu().numpy()[rows], Ow)
+    return res, po
+
+
+def test_full_size_wan14b_row_sample():
+    """BASELINE.json configs[2] (N = 75600, per-head outlier pairs with magnitudes U(5,25)), heads 0 and 17."""
+    _full_size_case(syn.WAN_14B, [0, 17])
+
+
+def test_full_size_hunyuan_row_sample_with_text_tokens():
+    """BASELINE.json configs[3] (N = 118800 video + 256 text tokens without RoPE, split 8/28/28), heads 3 and 11."""
+    _full_size_case(syn.HUNYUAN, [3, 11])
+
+
+def test_sweep_largest_n_and_naive_mode():
+    """BASELINE.json configs[4]: the largest sweep point (N = 131072) in the headline mode, and the naive
+    symmetric-INT4 / no-rotation baseline (NONE + SYM7) at N = 16384."""
+    _full_size_case(syn.SWEEP[4], [1], n_tiles=2)
+    _full_size_case(syn.SWEEP[1], [2], p_mode=orc.P_SYM7, rot_mode=orc.ROT_NONE, n_tiles=2)
+
+
+def test_mixed_precision_step_head_split():
+    """configs[4] schedule step: FP16 fallback on a head subset, INT4 on the rest, both through head_sel into one O."""
+    api = _api()
+    w = syn.small_variant(syn.SWEEP[0], (4, 16, 16), H=5)          # N = 1024
+    q, k, v = syn.gen_all(w)
+    res = api.run_int4(w, q, k, v, rot_mode=orc.ROT_HALF, want_fp16=True)
+    b, p = res['buffers'], res['p']
+    pol = dict(n_steps=50, n_blocks=1, first_steps=5, last_steps=0, first_blocks=0, last_blocks=0, fp16_head_mask=[0, 1, 0, 0, 1])
+    i4, f16 = api.rotattn_policy_split_heads(pol, 7, 0, w.B, w.H)
+    assert i4.tolist() == [0, 2, 3] and f16.tolist() == [1, 4]
+    O = torch.full_like(b.O, 9.0)
+    api.rotattn_fwd_int4(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, O, b.ws, api.WS_HAS_QK | api.WS_HAS_V,
+                         head_sel=torch.from_numpy(i4).cuda())
+    api.rotattn_fwd_fp16(p, b.Q16, b.K16, res['V'], O, b.ws16, head_sel=torch.from_numpy(f16).cuda())
+    torch.cuda.synchronize()
+    for h in range(w.H):
+        want = b.O16[0, h] if h in (1, 4) else b.O[0, h]
+        assert torch.equal(O[0, h], want)
+    i4, f16 = api.rotattn_policy_split_heads(pol, 2, 0, w.B, w.H)   # inside the first 5 steps: everything FP16
+    assert len(i4) == 0 and f16.tolist() == [0, 1, 2, 3, 4]
