@@ -92,6 +92,81 @@ def cpu_oracle_sample(n_rows=1024, threads=None):
     return dt, 4.0 * len(rows) * w.N * w.D, len(rows)
 
 
+def _time_ms(torch, fn, iters, warm=1):
+    for _ in range(warm):
+        fn()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(iters):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / iters
+
+
+def quality_report(api, syn, torch, w, Q, K, V, b, coef):
+    """Quality of the INT4 path against exact attention, next to the naive symmetric-INT4 / no-rotation baseline
+    (north_star).  The exact reference here is the library's own FP16 kernel on the same inputs (within 2e-3 of fp64
+    attention, tests/test_gpu_fwd_fp16.py); everything runs on the GPU, heads 0..3 of the bench workload."""
+    def metrics(o, ref):
+        o, ref = o.double().flatten(), ref.double().flatten()
+        return {'cosine': float((o @ ref) / (o.norm() * ref.norm())), 'rel_l1': float((o - ref).abs().sum() / ref.abs().sum())}
+    H4 = min(4, w.H)
+    out = {}
+    sl = lambda t: t[:, :H4].contiguous()
+    Qh, Kh, Vh = sl(Q), sl(K), sl(V)
+    ref = None
+    for name, rot, pm in (('half_asym15', api.ROT_HALF, api.P_ASYM15), ('interleaved_asym15', api.ROT_INTERLEAVED, api.P_ASYM15),
+                          ('none_asym15', api.ROT_NONE, api.P_ASYM15), ('naive_none_sym7', api.ROT_NONE, api.P_SYM7)):
+        p = api.params_for(w, rot, pm, H=H4)
+        cf = torch.from_numpy(api.rotattn_build_tables(p)).cuda()
+        bb = api.Buffers(p, want_fp16=ref is None)
+        api.rotattn_prepare_qk(p, cf, None, Qh, Kh, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.Q16, bb.K16, bb.ws)
+        api.rotattn_quant_v(p, Vh, bb.V4, bb.Vs, bb.ws)
+        api.rotattn_fwd_int4(p, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.V4, bb.Vs, bb.O, bb.ws, api.WS_HAS_QK | api.WS_HAS_V)
+        if ref is None:
+            api.rotattn_fwd_fp16(p, bb.Q16, bb.K16, Vh, bb.O16, bb.ws16)
+            ref = bb.O16.clone()
+        torch.cuda.synchronize()
+        out[name] = metrics(bb.O, ref)
+    out['note'] = 'synthetic outlier inputs (stand-ins for Wan2.2 activations); paper reports video-level metrics only (Table 1)'
+    return out
+
+
+def sweep_report(api, syn, torch):
+    """BASELINE.json configs[4]: H=24, D=128, N in {4096..131072}; per-N kernel ms / TOPS and the blended per-step time of
+    a 50-step schedule with the FP16 fallback on the first 5 steps and on round(0.1 H) seeded heads."""
+    rows = []
+    for w in syn.SWEEP:
+        p = api.params_for(w, api.ROT_HALF)
+        B, H, N, D = w.B, w.H, w.N, w.D
+        g = torch.Generator(device='cuda').manual_seed(w.seed)
+        Q, K, V = (torch.randn((B, H, N, D), device='cuda', dtype=torch.float16, generator=g) for _ in range(3))
+        cf = torch.from_numpy(api.rotattn_build_tables(p)).cuda()
+        bb = api.Buffers(p, want_fp16=True)
+        rng = np.random.Generator(np.random.PCG64(w.seed + 2))
+        f16_heads = np.sort(rng.choice(H, size=max(1, round(0.1 * H)), replace=False)).astype(np.int32)
+        i4_heads = np.array([h for h in range(H) if h not in set(f16_heads.tolist())], dtype=np.int32)
+        sel16, sel4 = torch.from_numpy(f16_heads).cuda(), torch.from_numpy(i4_heads).cuda()
+        it = 3 if N >= 65536 else 10
+        ws_state = api.WS_HAS_QK | api.WS_HAS_V
+        t_prep = _time_ms(torch, lambda: api.rotattn_prepare_qk(p, cf, None, Q, K, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.Q16, bb.K16, bb.ws), it)
+        t_qv = _time_ms(torch, lambda: api.rotattn_quant_v(p, V, bb.V4, bb.Vs, bb.ws), it)
+        t_i4 = _time_ms(torch, lambda: api.rotattn_fwd_int4(p, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.V4, bb.Vs, bb.O, bb.ws, ws_state), it)
+        t_f16 = _time_ms(torch, lambda: api.rotattn_fwd_fp16(p, bb.Q16, bb.K16, V, bb.O16, bb.ws16), it)
+        t_i4s = _time_ms(torch, lambda: api.rotattn_fwd_int4(p, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.V4, bb.Vs, bb.O, bb.ws, ws_state, head_sel=sel4), it)
+        t_f16s = _time_ms(torch, lambda: api.rotattn_fwd_fp16(p, bb.Q16, bb.K16, V, bb.O, bb.ws16, head_sel=sel16), it)
+        ops = 4.0 * B * H * N * N * D
+        blended = (5 * (t_prep + t_f16) + 45 * (t_prep + t_qv + t_i4s + t_f16s)) / 50
+        rows.append({'N': N, 'prepare_qk_ms': t_prep, 'quant_v_ms': t_qv, 'fwd_int4_ms': t_i4, 'fwd_int4_tops': ops / t_i4 / 1e9,
+                     'fwd_fp16_ms': t_f16, 'fwd_fp16_tflops': ops / t_f16 / 1e9, 'int4_heads': len(i4_heads), 'fp16_heads': len(f16_heads),
+                     'fwd_int4_subset_ms': t_i4s, 'fwd_fp16_subset_ms': t_f16s, 'blended_step_ms': blended, 'all_fp16_step_ms': t_prep + t_f16})
+        del Q, K, V, bb
+        torch.cuda.empty_cache()
+    return rows
+
+
 def run_reference(args):
     rank = int(os.environ.get('RANK', '0'))
     if rank != 0:
@@ -121,6 +196,7 @@ def main():
     ap.add_argument('--warmup', type=int, default=3)
     ap.add_argument('--impl', default='ours')
     ap.add_argument('--no-cpu-baseline', action='store_true')
+    ap.add_argument('--no-extras', action='store_true', help='skip the quality report and the N sweep (configs[4])')
     args = ap.parse_args()
     if args.impl == 'reference':
         return run_reference(args)
@@ -236,6 +312,11 @@ def main():
             dist.destroy_process_group()
         return
     pk = _peaks()
+    quality = sweep = None
+    if not args.no_extras and world == 1:
+        quality = quality_report(api, syn, torch, w, Q, Kt, V, b, coef)
+        del hq, hk, hv, hO
+        sweep = sweep_report(api, syn, torch)
     int8_peak = 2.0 * pk['bf16']      # dense int8 = 2x bf16 nominal ratio (4.5 / 2.25 PFLOP/s) applied to the measured bf16 peak
     achieved = ops / (t_int4 * 1e-3) / 1e12
     traffic = None
@@ -265,6 +346,10 @@ def main():
         'clocks': clocks,
         'paper_context': 'paper: up to 2.2x INT4 vs its FP16 kernel on A10, 1.68x end to end (PAPER.md:L267) - other hardware',
     }
+    if quality is not None:
+        out['quality_vs_own_fp16_kernel'] = quality
+    if sweep is not None:
+        out['sweep_mixed_precision'] = sweep
     if not args.no_cpu_baseline and world == 1:
         dt, cops, nrows = cpu_oracle_sample(4096)
         out['cpu_baseline'] = {'value': cops / dt / 1e12, 'unit': 'TOPS', 'cores': os.cpu_count(), 'kind': 'oracle', 'seconds': dt,
