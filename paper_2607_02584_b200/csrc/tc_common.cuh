@@ -55,6 +55,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   uint32_t spins = 0;
 #pragma unroll 1
   while (!mbar_try_wait(bar, parity)) {
+#ifdef ROTATTN_BACKOFF_ALL_NS
+    __nanosleep(ROTATTN_BACKOFF_ALL_NS);
+#endif
     if (++spins > (1u << 26)) __trap();
   }
 }
