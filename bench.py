@@ -351,7 +351,7 @@ def main():
     if sweep is not None:
         out['sweep_mixed_precision'] = sweep
     if not args.no_cpu_baseline and world == 1:
-        dt, cops, nrows = cpu_oracle_sample(4096)
+        dt, cops, nrows = cpu_oracle_sample(16384)
         out['cpu_baseline'] = {'value': cops / dt / 1e12, 'unit': 'TOPS', 'cores': os.cpu_count(), 'kind': 'oracle', 'seconds': dt,
                                'sample': f'{WORKLOAD}: 1 head, full prologue on N={N} tokens + O-quant for {nrows} query rows x all keys'}
     print(json.dumps(out))
