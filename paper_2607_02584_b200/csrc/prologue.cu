@@ -230,7 +230,7 @@ __global__ void __launch_bounds__(256, 2) prepare_qk_kernel(const PrepArgs a) {
 // through a swizzled shared tile, as int8 [D, npad] (K-major B operand of the P~V MMA).
 // ------------------------------------------------------------------------------------------------
 template <int D>
-__global__ void __launch_bounds__(256, 3) quant_v_kernel(const __half* __restrict__ V, uint8_t* __restrict__ V4,
+__global__ void __launch_bounds__(256, 4) quant_v_kernel(const __half* __restrict__ V, uint8_t* __restrict__ V4,
                                                       float* __restrict__ Vs, int8_t* __restrict__ V8T,
                                                       int N, int nG, int npad) {
   constexpr int CR = D / 8;           // 16-byte chunks per row
@@ -252,19 +252,23 @@ __global__ void __launch_bounds__(256, 3) quant_v_kernel(const __half* __restric
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
       int row = (q0 + ps * QPP) * 4 + r;
-      raw[ps][r] = (row0 + row < N) ? __ldg(reinterpret_cast<const uint4*>(base + (long long)row * D)) : make_uint4(0, 0, 0, 0);
+      raw[ps][r] = (row0 + row < N) ? __ldcs(reinterpret_cast<const uint4*>(base + (long long)row * D)) : make_uint4(0, 0, 0, 0);
     }
-  float am[8];
+  // per-channel amax over this thread's 16 rows on packed halves (max of |fp16| is exact), then across the CTA
+  __half2 am2[4];
 #pragma unroll
-  for (int j = 0; j < 8; ++j) am[j] = 0.f;
+  for (int k = 0; k < 4; ++k) am2[k] = __floats2half2_rn(0.f, 0.f);
 #pragma unroll
   for (int ps = 0; ps < NPASS; ++ps)
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
-      const __half* h = reinterpret_cast<const __half*>(&raw[ps][r]);
+      const __half2* h2 = reinterpret_cast<const __half2*>(&raw[ps][r]);
 #pragma unroll
-      for (int j = 0; j < 8; ++j) am[j] = fmaxf(am[j], fabsf(__half2float(h[j])));
+      for (int k = 0; k < 4; ++k) am2[k] = __hmax2(am2[k], __habs2(h2[k]));
     }
+  float am[8];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) { am[2 * k] = __low2float(am2[k]); am[2 * k + 1] = __high2float(am2[k]); }
 #pragma unroll
   for (int o = CR; o < 32; o <<= 1)
 #pragma unroll
@@ -283,35 +287,52 @@ __global__ void __launch_bounds__(256, 3) quant_v_kernel(const __half* __restric
     inv[j] = m > 0.f ? __fdiv_rn(7.0f, m) : 0.f;
     if (t < CR) Vs[(bh * nG + g) * D + cc * 8 + j] = __fdiv_rn(m, 7.0f);
   }
+  // code = rne(v * inv) in [-7,7] without clamping (|v| <= amax, inv = rn(7/amax)); q + 1.5*2^23 holds the two's-
+  // complement code in its low byte, |q| + 1.5*2^23 the magnitude; the sign of the code is the sign bit of the fp16 input.
 #pragma unroll
   for (int ps = 0; ps < NPASS; ++ps) {
-    uint32_t tw[8];
-#pragma unroll
-    for (int j = 0; j < 8; ++j) tw[j] = 0;
+    uint32_t fa[4][8];
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
-      const __half* h = reinterpret_cast<const __half*>(&raw[ps][r]);
-      uint32_t pk = 0;
+      const __half2* h2 = reinterpret_cast<const __half2*>(&raw[ps][r]);
+      uint32_t nb[4];
 #pragma unroll
-      for (int j = 0; j < 8; ++j) {
-        int c = quant_code(__half2float(h[j]), inv[j]);
-        pk |= (uint32_t)(c & 0xF) << (4 * j);
-        tw[j] |= code_byte(c) << (8 * r);
+      for (int k = 0; k < 4; ++k) {
+        const float2 x = __half22float2(h2[k]);
+        const float qa = __fmul_rn(x.x, inv[2 * k]), qb = __fmul_rn(x.y, inv[2 * k + 1]);
+        const uint32_t sa = __float_as_uint(__fadd_rn(qa, 12582912.f)), sb = __float_as_uint(__fadd_rn(qb, 12582912.f));
+        fa[r][2 * k] = __float_as_uint(__fadd_rn(fabsf(qa), 12582912.f));
+        fa[r][2 * k + 1] = __float_as_uint(__fadd_rn(fabsf(qb), 12582912.f));
+        nb[k] = (sa & 0xFu) | ((sb << 4) & 0xF0u);
       }
+      const uint32_t pk = __byte_perm(__byte_perm(nb[0], nb[1], 0x0040), __byte_perm(nb[2], nb[3], 0x0040), 0x5410);
       int row = (q0 + ps * QPP) * 4 + r;
       if (row0 + row < N) *reinterpret_cast<uint32_t*>(V4 + (bh * N + row0 + row) * (long long)(D / 2) + cc * 4) = pk;
     }
     if (V8T) {
       const int word = q0 + ps * QPP;
 #pragma unroll
-      for (int j = 0; j < 8; ++j) tileT[cc * 8 + j][(word ^ (SW * cc)) & 31] = tw[j];
+      for (int j = 0; j < 8; ++j) {
+        // operand byte of (row r, channel j) = magnitude | sign (only where the magnitude is non-zero: no -0 byte)
+        const uint32_t mag = __byte_perm(__byte_perm(fa[0][j], fa[1][j], 0x0040), __byte_perm(fa[2][j], fa[3][j], 0x0040), 0x5410);
+        const uint32_t* w0 = reinterpret_cast<const uint32_t*>(&raw[ps][0]);
+        const uint32_t* w1 = reinterpret_cast<const uint32_t*>(&raw[ps][1]);
+        const uint32_t* w2 = reinterpret_cast<const uint32_t*>(&raw[ps][2]);
+        const uint32_t* w3 = reinterpret_cast<const uint32_t*>(&raw[ps][3]);
+        const uint32_t sel = (j & 1) ? 0x0073u : 0x0051u;          // byte 3 (odd channel) / byte 1 (even channel) of the half2 word
+        const uint32_t sgn = __byte_perm(__byte_perm(w0[j >> 1], w1[j >> 1], sel), __byte_perm(w2[j >> 1], w3[j >> 1], sel), 0x5410);
+        const uint32_t nz = (mag + 0x7F7F7F7Fu) & 0x80808080u;
+        tileT[cc * 8 + j][(word ^ (SW * cc)) & 31] = mag | (sgn & nz);
+      }
     }
   }
   if (V8T) {
     __syncthreads();
-    for (int ch = warp; ch < D; ch += 8) {
-      uint32_t w = tileT[ch][(lane ^ (SW * (ch / 8))) & 31];
-      *reinterpret_cast<uint32_t*>(V8T + (bh * D + ch) * (long long)npad + row0 + lane * 4) = w;
+    int8_t* dst = V8T + (bh * D + warp) * (long long)npad + row0 + lane * 4;
+#pragma unroll
+    for (int i = 0; i < D / 8; ++i) {                       // channel ch = warp + 8 i
+      const int ch = warp + 8 * i;
+      *reinterpret_cast<uint32_t*>(dst + (long long)(8 * i) * npad) = tileT[ch][(lane ^ (SW * (ch / 8))) & 31];
     }
   }
 }
