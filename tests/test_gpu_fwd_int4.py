@@ -208,3 +208,33 @@ def test_mixed_precision_step_head_split():
         assert torch.equal(O[0, h], want)
     i4, f16 = api.rotattn_policy_split_heads(pol, 2, 0, w.B, w.H)   # inside the first 5 steps: everything FP16
     assert len(i4) == 0 and f16.tolist() == [0, 1, 2, 3, 4]
+
+
+@pytest.mark.parametrize('p_mode', [orc.P_ASYM15, orc.P_SYM7])
+def test_d128_running_normaliser_ragged(p_mode):
+    """p_norm = RUNNING (the other reading of Eq.12's normaliser) at D = 128 over several ragged tiles."""
+    api = _api()
+    w = syn.small_variant(syn.HUNYUAN, (3, 9, 13), n_text=21, H=2)
+    q, k, v = syn.gen_all(w)
+    res = api.run_int4(w, q, k, v, rot_mode=orc.ROT_HALF, p_mode=p_mode, p_norm=orc.NORM_RUNNING)
+    torch.cuda.synchronize()
+    po = orc.Params(w.B, w.H, w.N, w.D, w.grid, w.pairs, rot_mode=orc.ROT_HALF, p_mode=p_mode, p_norm=orc.NORM_RUNNING)
+    for h in range(w.H):
+        for qt in range(3):
+            _check_tile(api, res, po, 0, h, qt, p_mode, orc.NORM_RUNNING)
+
+
+def test_batch_of_two_and_d64_many_tiles():
+    """B = 2 (unit index = b * H + h) and D = 64 over 9 KV blocks with a ragged tail."""
+    api = _api()
+    from dataclasses import replace
+    w = replace(syn.small_variant(syn.TINY, (4, 16, 17), H=2), B=2)      # N = 1088 = 8 * 128 + 64
+    q, k, v = syn.gen_all(w)
+    res = api.run_int4(w, q, k, v, rot_mode=orc.ROT_INTERLEAVED)
+    torch.cuda.synchronize()
+    po = orc.Params(w.B, w.H, w.N, w.D, w.grid, w.pairs, rot_mode=orc.ROT_INTERLEAVED)
+    for bi in range(2):
+        for h in range(2):
+            qc, qs, kc, ks, vc, vs = _oracle_inputs(res, bi, h)
+            _check_o(res['O'][bi, h].float().cpu().numpy(), orc.o_quant(po, qc, qs, kc, ks, vc, vs))
+    _check_tile(api, res, po, 1, 1, 8, orc.P_ASYM15, orc.NORM_ROWBLOCK)
