@@ -23,6 +23,7 @@
 // (PAPER.md:L157 online softmax, L190 per-group V scales), so P~V cannot accumulate across blocks in tensor memory.
 #include <cmath>
 #include <cstdio>
+#include <type_traits>
 #include "fwd_int4.cuh"
 
 namespace rotattn {
@@ -308,25 +309,27 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       // ---- pass 1: t = S * ks (written back over S), block row max over this half
       float mx0 = -INFINITY, mx1 = -INFINITY;
       tmem_ld16(s_addr, va);
+      auto pass1 = [&](auto masked) {                    // one branch per block on the ragged case, not one per chunk
 #pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        tmem_wait_ld();
-        uint32_t(&cur)[16] = (c & 1) ? vb : va;
-        uint32_t(&nxt)[16] = (c & 1) ? va : vb;
-        if (c < 3) tmem_ld16(s_addr + (c + 1) * 16, nxt);
-        if (DEBUG) {
+        for (int c = 0; c < 4; ++c) {
+          tmem_wait_ld();
+          uint32_t(&cur)[16] = (c & 1) ? vb : va;
+          uint32_t(&nxt)[16] = (c & 1) ? va : vb;
+          if (c < 3) tmem_ld16(s_addr + (c + 1) * 16, nxt);
+          if (DEBUG) {
 #pragma unroll
-          for (int i = 0; i < 16; ++i)
-            a.S_dump[(size_t)r * a.npad + j * kTile + cb + c * 16 + i] = (int32_t)(__uint_as_float(cur[i]) * kAccScale);
-        }
+            for (int i = 0; i < 16; ++i)
+              a.S_dump[(size_t)r * a.npad + j * kTile + cb + c * 16 + i] = (int32_t)(__uint_as_float(cur[i]) * kAccScale);
+          }
 #if defined(ROTATTN_ABL) && (ROTATTN_ABL == 3 || ROTATTN_ABL == 6)      // development ablation: no pass-1 arithmetic / write-back
-        mx0 = fmaxf(mx0, __uint_as_float(cur[0]));
+          mx0 = fmaxf(mx0, __uint_as_float(cur[0]));
 #else
-        if (ragged) chunk_scale_max<true>(cur, ks2 + c * 8, nvalid - c * 16, tt, mx0, mx1);
-        else chunk_scale_max<false>(cur, ks2 + c * 8, 16, tt, mx0, mx1);
-        tmem_st16(s_addr + c * 16, tt);
+          chunk_scale_max<decltype(masked)::value>(cur, ks2 + c * 8, nvalid - c * 16, tt, mx0, mx1);
+          tmem_st16(s_addr + c * 16, tt);
 #endif
-      }
+        }
+      };
+      if (ragged) pass1(std::true_type{}); else pass1(std::false_type{});
       ROTATTN_STAMP(j, 1);
       float tmax = fmaxf(mx0, mx1);
       float* mxbuf = sMx + ((g * 2 + (n & 1)) * 2) * 128;
