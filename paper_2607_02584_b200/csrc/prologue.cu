@@ -84,25 +84,27 @@ __global__ void __launch_bounds__(256, 2) prepare_qk_kernel(const PrepArgs a) {
     // ---- load phase: TOK tokens x (Q, K) + their coefficient rows, all independent
     float4 A[TOK][PPL];
     __half hx[TOK][2][CPL];
+    const bool full = n0 + TOK <= a.N;                     // warp-uniform: no per-token guards on the common path
+    const __half* src0 = a.X[0] + (head0 + n0) * D + lane * CPL;
+    const __half* src1 = a.X[1] + (head0 + n0) * D + lane * CPL;
 #pragma unroll
     for (int t = 0; t < TOK; ++t) {
       const int n = n0 + t;
-      if (n < a.N) {
-        const long long tok = head0 + n;
-#pragma unroll
-        for (int m = 0; m < 2; ++m) {
-          const __half* src = a.X[m] + tok * D + lane * CPL;
-          if (CPL == 4) *reinterpret_cast<uint2*>(hx[t][m]) = __ldcs(reinterpret_cast<const uint2*>(src));
-          else *reinterpret_cast<uint32_t*>(hx[t][m]) = __ldcs(reinterpret_cast<const uint32_t*>(src));
-        }
-        int pos[3];
-        if (n < a.n_rope) {
-          pos[0] = pt; pos[1] = ph; pos[2] = pw;
+      if (full || n < a.N) {
+        if (CPL == 4) {
+          *reinterpret_cast<uint2*>(hx[t][0]) = __ldcs(reinterpret_cast<const uint2*>(src0 + t * D));
+          *reinterpret_cast<uint2*>(hx[t][1]) = __ldcs(reinterpret_cast<const uint2*>(src1 + t * D));
         } else {
-          pos[0] = a.gt; pos[1] = a.gh; pos[2] = a.gw;     // no-RoPE rows
+          *reinterpret_cast<uint32_t*>(hx[t][0]) = __ldcs(reinterpret_cast<const uint32_t*>(src0 + t * D));
+          *reinterpret_cast<uint32_t*>(hx[t][1]) = __ldcs(reinterpret_cast<const uint32_t*>(src1 + t * D));
         }
+        const bool rope = n < a.n_rope;                    // text tokens use the no-RoPE rows of the table
+        const int p0 = rope ? pt : a.gt, p1 = rope ? ph : a.gh, p2 = rope ? pw : a.gw;
 #pragma unroll
-        for (int i = 0; i < PPL; ++i) A[t][i] = __ldg(a.coef + cbase[i] + pos[caxis[i]] * cstride[i]);
+        for (int i = 0; i < PPL; ++i) {
+          const int pos = caxis[i] == 0 ? p0 : (caxis[i] == 1 ? p1 : p2);
+          A[t][i] = __ldg(a.coef + cbase[i] + pos * cstride[i]);
+        }
       }
       if (++pw == a.gw) { pw = 0; if (++ph == a.gh) { ph = 0; ++pt; } }
     }
@@ -166,6 +168,7 @@ __global__ void __launch_bounds__(256, 2) prepare_qk_kernel(const PrepArgs a) {
       if (lane < 2 * TOK) {
         my_scale = __fdiv_rn(am, 7.0f);
         my_inv = am > 0.f ? __fdiv_rn(7.0f, am) : 0.f;
+        if (n0 + (lane >> 1) < a.N) a.Xs[lane & 1][head0 + n0 + (lane >> 1)] = my_scale;     // lane 2 t + m owns (token t, tensor m)
       }
     }
 #pragma unroll
@@ -174,7 +177,6 @@ __global__ void __launch_bounds__(256, 2) prepare_qk_kernel(const PrepArgs a) {
       const long long tok = head0 + n0 + t;
 #pragma unroll
       for (int m = 0; m < 2; ++m) {
-        const float scale = __shfl_sync(0xffffffffu, my_scale, 2 * t + m);
         const float inv = __shfl_sync(0xffffffffu, my_inv, 2 * t + m);
         // code = rne(y * inv) is in [-7,7] without clamping (|y| <= amax and inv = rn(7/amax) give |y*inv| < 7.5).
         // fs = q + 1.5*2^23 holds the two's-complement code in its low byte, fa = |q| + 1.5*2^23 the magnitude.
@@ -192,7 +194,6 @@ __global__ void __launch_bounds__(256, 2) prepare_qk_kernel(const PrepArgs a) {
         } else {
           a.X4[m][tok * (D / 2) + lane] = (uint8_t)((fs[0] & 0xFu) | ((fs[1] << 4) & 0xF0u));
         }
-        if (lane == 0) a.Xs[m][tok] = scale;
         if (a.X8[m]) {
           // sign-magnitude operand bytes (code_byte): magnitude bytes | sign bits of q (a zero code has q = +-0 or |q| < 0.5:
           // its sign must not be stored, hence the mask with the non-zero test folded into the magnitude: -0 byte is avoided
