@@ -149,6 +149,9 @@ fwd_fp16_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 #pragma unroll
         for (int x = 0; x < 2; ++x) {
           if (j > 0) mbar_wait(&pv_done[x], (j - 1) & 1);              // P_X(j-1), which aliases S_X, has been consumed
+          // Stagger the two tiles by one softmax: tile 1 starts when tile 0 has left its first exp2 phase, so that from
+          // then on one tile is in its softmax (MUFU) while the tensor pipe works for the other one.
+          if (j == 0 && x == 1) mbar_wait(&p_full[0], 0);
           tc_fence_after();
           if (elect_one()) {
             const uint32_t q_addr = smem_u32(sQ + x * L::Q_BYTES), k_addr = smem_u32(sK + st * L::K_BYTES);
