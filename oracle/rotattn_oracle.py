@@ -23,8 +23,9 @@ operation, no fused multiply-add (NumPy never contracts), so INT4 codes are
 reproducible bit for bit.  Softmax arithmetic is fp64.
 
 Pins: tests/test_oracle_pins.py (-m "not gpu").  Parity status per function:
-  hadamard, h2, rope, coef_table, apply_rope_rot, quantisers, pack/unpack, integer
-  products, P codes, online softmax, policy : pinned (see that file).
+  hadamard, h2, token_positions (golden triples on an asymmetric grid), rope, coef_table,
+  apply_rope_rot, quantisers, pack/unpack, integer products, P codes, online softmax,
+  policy : pinned (see that file).
   INT4-vs-exact *quality numbers* : parity unpinned (paper gives only video-level
   metrics on real weights, Table 1); reported, never asserted.
 """

@@ -113,15 +113,27 @@ def gen_head(w: Workload, b: int, h: int):
     return q.astype(np.float16), k.astype(np.float16), v.astype(np.float16)
 
 
-def gen_all(w: Workload, heads=None):
-    """fp16 [B,H',N,D] for the selected heads (default all)."""
+def gen_all(w: Workload, heads=None, workers=None):
+    """fp16 [B,H',N,D] for the selected heads (default all).  Every (b,h) has its own generator, so the heads are
+    drawn by a small thread pool without changing any value."""
+    from concurrent.futures import ThreadPoolExecutor
     heads = list(range(w.H)) if heads is None else list(heads)
     q = np.empty((w.B, len(heads), w.N, w.D), dtype=np.float16)
     k = np.empty_like(q)
     v = np.empty_like(q)
-    for b in range(w.B):
-        for i, h in enumerate(heads):
-            q[b, i], k[b, i], v[b, i] = gen_head(w, b, h)
+
+    def one(bi):
+        b, i = bi
+        q[b, i], k[b, i], v[b, i] = gen_head(w, b, heads[i])
+
+    units = [(b, i) for b in range(w.B) for i in range(len(heads))]
+    workers = min(8, len(units)) if workers is None else workers
+    if workers <= 1:
+        for u in units:
+            one(u)
+    else:
+        with ThreadPoolExecutor(workers) as ex:
+            list(ex.map(one, units))
     return q, k, v
 
 

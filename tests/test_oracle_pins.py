@@ -16,8 +16,13 @@ from synth import video_qkv as syn
 GOLD = os.path.join(os.path.dirname(__file__), 'golden')
 
 
+GRID = (4, 6, 10)          # Hh != W and P_h != P_w below: none of the pins is symmetric in the h and w axes
+PAIRS = (12, 9, 11)
+N0 = GRID[0] * GRID[1] * GRID[2]
+
+
 def _params(rot_mode=orc.ROT_HALF, **kw):
-    base = dict(B=1, H=1, N=4 * 8 * 8, D=64, grid=(4, 8, 8), pairs=(12, 10, 10), rot_mode=rot_mode)
+    base = dict(B=1, H=1, N=N0, D=64, grid=GRID, pairs=PAIRS, rot_mode=rot_mode)
     base.update(kw)
     return orc.Params(**base)
 
@@ -74,6 +79,19 @@ def test_hadamard_recursion_and_library(n):
     assert np.allclose((V @ H) @ H.T, V, atol=1e-12)                         # Eq.14
 
 
+# ---------------------------------------------------------------- token <-> position (reading 4)
+def test_token_positions_golden_asymmetric_grid():
+    rows = _read_rows('token_positions_2x3x5.txt')
+    t, h, w, is_rope = orc.token_positions(31, (2, 3, 5))
+    for n, gt, gh, gw, gr in ((int(x) for x in r) for r in rows):
+        assert (int(t[n]), int(h[n]), int(w[n]), int(is_rope[n])) == (gt, gh, gw, gr), n
+    # the library's row-major unravel is the same map (w fastest) on every video token of a second asymmetric grid
+    t, h, w, is_rope = orc.token_positions(N0 + 2, GRID)
+    ut, uh, uw = np.unravel_index(np.arange(N0), GRID)
+    assert np.array_equal(t[:N0], ut) and np.array_equal(h[:N0], uh) and np.array_equal(w[:N0], uw)
+    assert is_rope[:N0].all() and not is_rope[N0:].any()
+
+
 # ---------------------------------------------------------------- RoPE (L58-62)
 def test_rope_textbook_properties():
     p = _params()
@@ -86,8 +104,8 @@ def test_rope_textbook_properties():
     ny = y[:, 0::2] ** 2 + y[:, 1::2] ** 2
     assert np.allclose(nx, ny, rtol=1e-12)
     # complex-number formulation: (x0 + i x1) e^{i theta}
-    t, h, w, _ = orc.token_positions(p.N, p.grid)
-    pos = np.concatenate([np.repeat(t[:, None], 12, 1), np.repeat(h[:, None], 10, 1), np.repeat(w[:, None], 10, 1)], axis=1)
+    t, h, w = np.unravel_index(np.arange(p.N), p.grid)       # library row-major map, not the oracle's own
+    pos = np.concatenate([np.repeat(x[:, None], P, 1) for x, P in zip((t, h, w), p.pairs)], axis=1)
     fr = np.concatenate([10000.0 ** (-np.arange(P) / P) for P in p.pairs])
     z = (x[:, 0::2] + 1j * x[:, 1::2]) * np.exp(1j * pos * fr[None, :])
     assert np.allclose(y[:, 0::2], z.real, atol=1e-10) and np.allclose(y[:, 1::2], z.imag, atol=1e-10)
@@ -145,7 +163,7 @@ def test_merged_table_equals_sequential_and_closed_form():
 
 @pytest.mark.parametrize('mode', [orc.ROT_NONE, orc.ROT_INTERLEAVED, orc.ROT_HALF])
 def test_fp32_apply_matches_fp64(mode):
-    p = _params(mode, N=4 * 8 * 8 + 5)     # 5 text tokens without RoPE
+    p = _params(mode, N=N0 + 5)     # 5 text tokens without RoPE
     rng = np.random.default_rng(4)
     rot = _rand_o2(rng, p.D // 2)
     x16 = (rng.standard_normal((p.N, p.D)) * 3).astype(np.float16)
@@ -161,7 +179,7 @@ def test_fp32_apply_matches_fp64(mode):
 @pytest.mark.parametrize('mode', [orc.ROT_INTERLEAVED, orc.ROT_HALF])
 @pytest.mark.parametrize('randrot', [False, True])
 def test_qk_invariance_under_shared_rotation(mode, randrot):
-    p = _params(mode, N=4 * 8 * 8 + 3)
+    p = _params(mode, N=N0 + 3)
     rng = np.random.default_rng(5)
     rot = _rand_o2(rng, p.D // 2) if randrot else None
     q = rng.standard_normal((p.N, p.D))
@@ -179,7 +197,7 @@ def test_half_pairing_structure():
     assert np.array_equal(orc.dense_rotation(p, orc.ROT_HALF, ident), np.eye(p.D))
     R = orc.dense_rotation(p, orc.ROT_HALF)
     assert np.allclose(R @ R, np.eye(p.D), atol=1e-12)               # H_2^2 = I
-    # channel o_j + i couples only with o_j + i + D_j/2 (Eq.8): sections of 24, 20, 20 channels
+    # channel o_j + i couples only with o_j + i + D_j/2 (Eq.8): sections of 2 P_j channels
     nz = np.abs(R) > 0
     o = 0
     for P in p.pairs:
