@@ -27,16 +27,19 @@ extern "C" {
 typedef enum rotattn_status {
   ROTATTN_OK = 0,
   ROTATTN_ERR_INVALID_ARG = -1,         /* NULL pointer, sum(pairs) != D/2, t*h*w > N, n_sel out of range */
-  ROTATTN_ERR_UNSUPPORTED = -2,         /* D not in {64,128}, kv_block != 128, v_group != 128, qk_group != 1,
-                                           device is not sm_100 */
+  ROTATTN_ERR_UNSUPPORTED = -2,         /* D not in {64,128}, kv_block != 128, v_group != 128, qk_group not in {1,128},
+                                           p_norm = RUNNING or smooth with a non-default granularity, device is not sm_100 */
   ROTATTN_ERR_NOT_ORTHOGONAL = -3,      /* max|R_i^T R_i - I| > 1e-5 */
   ROTATTN_ERR_WORKSPACE_TOO_SMALL = -4,
   ROTATTN_ERR_CUDA = -5                 /* a CUDA runtime/driver call failed; see rotattn_last_cuda_error() */
 } rotattn_status;
 
-enum { ROTATTN_ROT_NONE = 0, ROTATTN_ROT_INTERLEAVED = 1, ROTATTN_ROT_HALF = 2 };
+enum { ROTATTN_ROT_NONE = 0, ROTATTN_ROT_INTERLEAVED = 1, ROTATTN_ROT_HALF = 2,
+       ROTATTN_ROT_FULL = 3 /* the paper's "Full" ablation baseline: dense D x D Hadamard after RoPE */ };
 enum { ROTATTN_P_ASYM15 = 0, ROTATTN_P_SYM7 = 1 };
 enum { ROTATTN_NORM_ROWBLOCK = 0, ROTATTN_NORM_RUNNING = 1 };
+enum { ROTATTN_VSCALE_CHANNEL = 0 /* one V scale per (128-token group, channel): DESIGN.md reading 11 */,
+       ROTATTN_VSCALE_GROUP = 1   /* one V scale per 128-token group */ };
 /* ws_state bits for rotattn_fwd_int4 */
 enum { ROTATTN_WS_HAS_QK = 1, ROTATTN_WS_HAS_V = 2 };
 
@@ -52,9 +55,13 @@ typedef struct rotattn_params {
                                          HALF (Eq.8, same register pass) */
   int32_t p_mode;                     /* ROTATTN_P_ASYM15 (Eq.12) | ROTATTN_P_SYM7 (Eq.11) */
   int32_t p_norm;                     /* ROTATTN_NORM_ROWBLOCK (reading 13, default) | ROTATTN_NORM_RUNNING */
-  int32_t qk_group;                   /* tokens per Q/K scale; 1 = per-token (L190).  Only 1 is built. */
+  int32_t qk_group;                   /* tokens per Q/K scale: 1 = per-token (L190, the paper's setting) or 128 = one scale
+                                         per 128-token block (north_star "per-block scales") */
   int32_t v_group;                    /* tokens per V scale group (L190, reading 11).  Only 128 is built. */
   int32_t kv_block;                   /* P-normalisation block (L157, reading 18).  Only 128 is built. */
+  int32_t v_scale;                    /* ROTATTN_VSCALE_CHANNEL (default) | ROTATTN_VSCALE_GROUP */
+  int32_t smooth;                     /* 0 | 1: subtract the token mean of Q, K, V before quantisation ("we first
+                                         perform smoothing on Q, K, V"; L40, L52), see rotattn_smooth_* below */
 } rotattn_params;
 
 /* ---- host-side helpers (no GPU needed) ------------------------------------------------------- */
@@ -75,18 +82,20 @@ size_t rotattn_table_floats(const rotattn_params* p);
  * Errors: INVALID_ARG, UNSUPPORTED, NOT_ORTHOGONAL. */
 int rotattn_build_tables(const rotattn_params* p, const float* rot_host, float* coef_host);
 
-/* Bytes of scratch the device entry points need.  which = 0: INT4 path (shared by prepare_qk,
- * quant_v and fwd_int4: widened int8 copies of the Q/K codes [B,H,N,D] and of the V codes
- * transposed [B,H,D,ceil128(N)]); which = 1: FP16 path (transposed V copy). */
+/* Bytes of scratch the device entry points need.  which = 0 (prepare_qk / quant_v / smooth_stats) and which = 1
+ * (fwd_int4) are one and the same INT4-path workspace: sign-magnitude operand bytes of the Q/K codes [B,H,N,128] and
+ * of the V codes transposed [B,H,D,ceil128(N)] (one byte per code = the E4M3 bit pattern of code * 2^-9), the key
+ * scales padded to whole blocks, and the smoothing state.  which = 2: FP16 path (transposed V copy). */
 size_t rotattn_workspace_bytes(const rotattn_params* p, int which);
 
 /* Mixed-precision fallback policy: FP16 on the first/last sampling steps and the
  * first/last DiT blocks (and on heads flagged in fp16_head_mask), INT4 elsewhere.  Pure host logic. */
 typedef struct rotattn_policy {
   int32_t n_steps, n_blocks, first_steps, last_steps, first_blocks, last_blocks;
-  const uint8_t* fp16_head_mask;      /* host [H] or NULL */
+  int32_t n_heads;                    /* entries of fp16_head_mask (ignored when the mask is NULL) */
+  const uint8_t* fp16_head_mask;      /* host [n_heads] or NULL */
 } rotattn_policy;
-/* 0 = INT4, 1 = FP16, negative = error. */
+/* 0 = INT4, 1 = FP16, negative = error (INVALID_ARG also for head >= n_heads when a mask is given). */
 int rotattn_policy_select(const rotattn_policy* pol, int32_t step, int32_t block, int32_t head);
 /* Fill sel_int4 / sel_fp16 (host int32, capacity B*H each) with the b*H+h indices each kernel must run
  * for this (step, block); counts are returned through n_int4 / n_fp16. */
@@ -107,10 +116,15 @@ const char* rotattn_last_cuda_error(void);
  * rot_dev : device float [D/2][4] blocks used by HALF mode, or NULL for H_2.  Ignored otherwise.
  * Q,K     : fp16 [B,H,N,D].
  * Q4,K4   : out, packed codes [B,H,N,D/2] uint8: byte i = (code_{2i} & 0xF) | (code_{2i+1} & 0xF) << 4.
- * Qs,Ks   : out, fp32 scales [B,H,N].
- * Qrope16,Krope16 : optional out (may be NULL), y rounded once to fp16 [B,H,N,D] (input of fwd_fp16).
- * workspace: optional (may be NULL): if given (>= rotattn_workspace_bytes(p,0)) the widened int8
- *           copies used by fwd_int4 are also written (then pass ROTATTN_WS_HAS_QK to fwd_int4). */
+ * Qs,Ks   : out, fp32 scales [B,H,N]  (qk_group = 128: one scale per 128-token block, [B,H,ceil(N/128)], amax over
+ *           the block's tokens and channels).
+ * Qrope16,Krope16 : optional out (may be NULL), y rounded once to fp16 [B,H,N,D] (input of fwd_fp16; never smoothed).
+ * rot_mode = FULL (the paper's "Full" baseline, L208): after RoPE, y <- y H_D / sqrt(D) as a Sylvester butterfly
+ *           (strides 1, 2, .., D/2; (a,b) -> (a+b, a-b); one multiplication by fl(1/sqrt(D)) at the end).
+ * smooth = 1: rotattn_smooth_stats must have run on this workspace first; y - mean_n(y) is quantised instead of y, and
+ *           the per-key correction mean(y_Q) . (y_K - mean(y_K)) is stored in the workspace for fwd_int4.
+ * workspace: optional (may be NULL, required for smooth): if given (>= rotattn_workspace_bytes(p,0)) the operand
+ *           bytes and padded key scales used by fwd_int4 are also written (then pass ROTATTN_WS_HAS_QK to fwd_int4). */
 int rotattn_prepare_qk(const rotattn_params* p, const float* coef_dev, const float* rot_dev,
                        const void* Q, const void* K,
                        uint8_t* Q4, float* Qs, uint8_t* K4, float* Ks,
@@ -120,52 +134,54 @@ int rotattn_prepare_qk(const rotattn_params* p, const float* coef_dev, const flo
 /* Step a3: per-group symmetric INT4 of Hadamard-domain V (L190; Eq.14: H is folded into
  * W_v offline, so V arrives transformed).  One scale per (128 consecutive tokens, channel); the ragged
  * last group uses the tokens that exist.
- * V : fp16 [B,H,N,D].  V4: out packed [B,H,N,D/2].  Vs: out fp32 [B,H,ceil(N/128),D].
+ * V : fp16 [B,H,N,D].  V4: out packed [B,H,N,D/2].  Vs: out fp32 [B,H,ceil(N/128),D], 16-byte aligned
+ *   (v_scale = GROUP: one scale per group, [B,H,ceil(N/128)], amax over the group's tokens and channels).
+ * smooth = 1: v - mean_n(v) is quantised (the mean is added back to O by fwd_int4).
  * workspace as for prepare_qk (then pass ROTATTN_WS_HAS_V to fwd_int4). */
 int rotattn_quant_v(const rotattn_params* p, const void* V, uint8_t* V4, float* Vs,
                     void* workspace, size_t ws_bytes, void* stream);
 
-/* Steps a4-a9: INT4 FlashAttention forward (§4.2).
- *   S = Q4 K4^T as an integer tensor-core MMA with int32 accumulation (L157);
+/* Smoothing pre-pass ("we first perform smoothing on Q, K, V", L40, L52): column means
+ * over the N tokens of y_Q, y_K (after RoPE and rotation) and of V, per (b,h), kept in the workspace.  Needed once
+ * before rotattn_prepare_qk / rotattn_quant_v when p->smooth = 1.  The sums are taken in fixed point (units of 2^-20
+ * for y, 2^-24 for the fp16 V) so that they do not depend on the order of summation:
+ *   mean = fl32( fp64(sum_n rne(y_n * 2^20)) / (N * 2^20) ).
+ * Exactness of the shifts: K - mean(K) leaves softmax(QK^T) unchanged; (Q - mean Q) K'^T + mean(Q) K'^T = Q K'^T, the
+ * rank-1 term is added to S in fp32; softmax(.)(V - mean V) + mean V = softmax(.) V. */
+int rotattn_smooth_stats(const rotattn_params* p, const float* coef_dev, const float* rot_dev,
+                         const void* Q, const void* K, const void* V,
+                         void* workspace, size_t ws_bytes, void* stream);
+/* Copies the smoothing state out of the workspace (either pointer may be NULL):
+ * means_out fp32 [B,H,3,D] (y_Q, y_K, V); kcorr_out fp32 [B,H,N] = mean(y_Q) . (y_K - mean y_K) * log2(e)/sqrt(D). */
+int rotattn_smooth_read(const rotattn_params* p, const void* workspace, size_t ws_bytes,
+                        float* means_out, float* kcorr_out, void* stream);
+
+/* Steps a4-a9: INT4 FlashAttention forward (PAPER.md 4.2 L155-170).
+ *   S = Q4 K4^T on the tensor cores with exact integer accumulation (L157): sm_100a has no 4-bit integer MMA and its
+ *   8-bit integer kind returns int32 that would have to be converted three times per element, so the codes travel as
+ *   the E4M3 bit patterns of code * 2^-9 through tcgen05 kind::f8f6f4 and the fp32 accumulators hold acc * 2^-18
+ *   exactly (|acc| <= 13440 < 2^24; adversarial tests in tests/test_gpu_probe.py).
  *   s_ij = acc * Qs_i * Ks_j / sqrt(D); per KV block of 128 keys: block row max, P^ = exp(s - max),
  *   u = rne(15 P^) in {0..15} (Eq.12: scale 15, zero-point -8, stored unsigned u = c + 8; SYM7: rne(7 P^));
- *   integer P~V with int32 accumulation; O <- alpha O + beta (Vs/15) pv in fp32; epilogue O/l -> fp16.
- * Q4..Vs: the outputs of prepare_qk / quant_v.   O: out fp16 [B,H,N,D] (only selected heads written).
+ *   integer P~V, same exact path; O <- alpha O + beta (Vs/15) pv in fp32; epilogue O/l -> fp16.
+ * Q4..Vs: the outputs of prepare_qk / quant_v (shapes follow qk_group / v_scale).
+ * O: out fp16 [B,H,N,D], 16-byte aligned (only selected heads written).
  * head_sel: device int32 [n_sel] of b*H+h indices to process, or NULL (all B*H heads, n_sel ignored).
- * workspace: required, >= rotattn_workspace_bytes(p,0).  ws_state: ROTATTN_WS_HAS_QK|ROTATTN_WS_HAS_V
+ * workspace: required, >= rotattn_workspace_bytes(p,1).  ws_state: ROTATTN_WS_HAS_QK|ROTATTN_WS_HAS_V
  *   if this workspace was passed to prepare_qk / quant_v with the same params; missing copies are rebuilt
- *   from the packed buffers by an unpack kernel first. */
+ *   from the packed buffers by an unpack kernel first (smooth = 1 needs both bits: its state exists only there). */
 int rotattn_fwd_int4(const rotattn_params* p,
                      const uint8_t* Q4, const float* Qs, const uint8_t* K4, const float* Ks,
                      const uint8_t* V4, const float* Vs, void* O,
                      const int32_t* head_sel, int32_t n_sel,
                      void* workspace, size_t ws_bytes, int32_t ws_state, void* stream);
 
-/* Same computation for ONE (bh, query tile of 128 rows), additionally dumping the int32 S accumulators
- * and the P codes (parity tests only; not on the timed path).
- * S_dump: int32 [128, ceil128(N)], P_dump: uint8 [128, ceil128(N)], O_tile: fp16 [128, D] (rows >= N untouched). */
-int rotattn_fwd_int4_debug(const rotattn_params* p,
-                           const uint8_t* Q4, const float* Qs, const uint8_t* K4, const float* Ks,
-                           const uint8_t* V4, const float* Vs,
-                           int32_t bh, int32_t q_tile, int32_t* S_dump, uint8_t* P_dump, void* O_tile,
-                           void* workspace, size_t ws_bytes, int32_t ws_state, void* stream);
-
 /* Step a10: FP16 FlashAttention forward, the fallback precision and the speed baseline (L21, L192, L267).
  * Q16,K16: fp16 RoPE'd Q,K [B,H,N,D] (Qrope16/Krope16 of prepare_qk); V16: fp16 V [B,H,N,D]; fp32 accumulate.
- * workspace: required, >= rotattn_workspace_bytes(p,1). */
+ * workspace: required, >= rotattn_workspace_bytes(p,2). */
 int rotattn_fwd_fp16(const rotattn_params* p, const void* Q16, const void* K16, const void* V16, void* O,
                      const int32_t* head_sel, int32_t n_sel,
                      void* workspace, size_t ws_bytes, void* stream);
-
-/* Measurement aid: dense 8-bit GEMM C[M,N] = A[M,K] * B[N,K]^T on the same tcgen05 path the attention
- * kernel uses; used to MEASURE the dense INT8 tensor peak that the roofline of fwd_int4 is quoted against.
- * M multiple of 128, N multiple of 256, K multiple of 128.  A,B: device, row-major, 1 byte per element.
- *   mode 0: kind::i8, A and B signed int8, C int32.
- *   mode 1: kind::f8f6f4, A and B E4M3 bit patterns, C float (fp32 accumulators).
- *   mode 2: kind::i8 with A (UNSIGNED u8) staged through tensor memory, B signed; M=N=K=128 only
- *           (checks the TMEM A-operand layout used for the P~V product), C int32. */
-int rotattn_probe_gemm8(int32_t M, int32_t N, int32_t K, const void* A, const void* B, void* C,
-                        int32_t mode, void* stream);
 
 #ifdef __cplusplus
 }

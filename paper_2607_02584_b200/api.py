@@ -8,8 +8,8 @@ import numpy as np
 import torch
 
 from . import binding as _b
-from .binding import (ROT_NONE, ROT_INTERLEAVED, ROT_HALF, P_ASYM15, P_SYM7, NORM_ROWBLOCK, NORM_RUNNING,
-                      WS_HAS_QK, WS_HAS_V, make_params, check)
+from .binding import (ROT_NONE, ROT_INTERLEAVED, ROT_HALF, ROT_FULL, P_ASYM15, P_SYM7, NORM_ROWBLOCK, NORM_RUNNING,
+                      WS_HAS_QK, WS_HAS_V, VSCALE_CHANNEL, VSCALE_GROUP, make_params, check)
 
 lib = _b.lib
 
@@ -52,23 +52,23 @@ def rotattn_workspace_bytes(p, which: int) -> int:
     return int(lib.rotattn_workspace_bytes(C.byref(p), which))
 
 
-def rotattn_policy_select(pol: dict, step: int, block: int, head: int = 0) -> int:
+def _policy_struct(pol: dict):
     mask = pol.get('fp16_head_mask')
     arr = None
     if mask is not None:
         arr = (C.c_uint8 * len(mask))(*[int(x) for x in mask])
     st = _b.RotattnPolicy(pol['n_steps'], pol['n_blocks'], pol['first_steps'], pol['last_steps'],
-                          pol['first_blocks'], pol['last_blocks'], arr)
+                          pol['first_blocks'], pol['last_blocks'], 0 if mask is None else len(mask), arr)
+    return st, arr          # arr is returned so that it stays alive while the struct points at it
+
+
+def rotattn_policy_select(pol: dict, step: int, block: int, head: int = 0) -> int:
+    st, _keep = _policy_struct(pol)
     return int(lib.rotattn_policy_select(C.byref(st), step, block, head))
 
 
 def rotattn_policy_split_heads(pol: dict, step: int, block: int, B: int, H: int):
-    mask = pol.get('fp16_head_mask')
-    arr = None
-    if mask is not None:
-        arr = (C.c_uint8 * len(mask))(*[int(x) for x in mask])
-    st = _b.RotattnPolicy(pol['n_steps'], pol['n_blocks'], pol['first_steps'], pol['last_steps'],
-                          pol['first_blocks'], pol['last_blocks'], arr)
+    st, _keep = _policy_struct(pol)
     a = np.zeros(B * H, dtype=np.int32)
     b = np.zeros(B * H, dtype=np.int32)
     na, nb = C.c_int32(0), C.c_int32(0)
@@ -102,11 +102,23 @@ def rotattn_fwd_int4(p, Q4, Qs, K4, Ks, V4, Vs, O, workspace, ws_state, head_sel
           'rotattn_fwd_int4')
 
 
+def rotattn_smooth_stats(p, coef_dev, rot_dev, Q, K, V, workspace, stream=None):
+    _need_cuda(coef_dev, rot_dev, Q, K, V, workspace)
+    check(lib.rotattn_smooth_stats(C.byref(p), _ptr(coef_dev), _ptr(rot_dev), _ptr(Q), _ptr(K), _ptr(V), _ptr(workspace),
+                                   workspace.numel() * workspace.element_size(), _stream(stream)), 'rotattn_smooth_stats')
+
+
+def rotattn_smooth_read(p, workspace, means_out=None, kcorr_out=None, stream=None):
+    _need_cuda(workspace, means_out, kcorr_out)
+    check(lib.rotattn_smooth_read(C.byref(p), _ptr(workspace), workspace.numel() * workspace.element_size(),
+                                  _ptr(means_out), _ptr(kcorr_out), _stream(stream)), 'rotattn_smooth_read')
+
+
 def rotattn_fwd_int4_debug(p, Q4, Qs, K4, Ks, V4, Vs, bh, q_tile, S_dump, P_dump, O_tile, workspace, ws_state,
-                           stream=None):
-    _need_cuda(Q4, Qs, K4, Ks, V4, Vs, S_dump, P_dump, O_tile, workspace)
+                           PV_dump=None, stream=None):
+    _need_cuda(Q4, Qs, K4, Ks, V4, Vs, S_dump, P_dump, PV_dump, O_tile, workspace)
     check(lib.rotattn_fwd_int4_debug(C.byref(p), _ptr(Q4), _ptr(Qs), _ptr(K4), _ptr(Ks), _ptr(V4), _ptr(Vs),
-                                     bh, q_tile, _ptr(S_dump), _ptr(P_dump), _ptr(O_tile), _ptr(workspace),
+                                     bh, q_tile, _ptr(S_dump), _ptr(P_dump), _ptr(PV_dump), _ptr(O_tile), _ptr(workspace),
                                      workspace.numel() * workspace.element_size(), ws_state, _stream(stream)),
           'rotattn_fwd_int4_debug')
 
@@ -134,9 +146,9 @@ class Buffers:
         self.Q4 = torch.empty((B, H, N, D // 2), dtype=u8, device=device)
         self.K4 = torch.empty_like(self.Q4)
         self.V4 = torch.empty_like(self.Q4)
-        self.Qs = torch.empty((B, H, N), dtype=f32, device=device)
+        self.Qs = torch.empty((B, H, N if p.qk_group == 1 else nG), dtype=f32, device=device)
         self.Ks = torch.empty_like(self.Qs)
-        self.Vs = torch.empty((B, H, nG, D), dtype=f32, device=device)
+        self.Vs = torch.empty((B, H, nG, D) if p.v_scale == VSCALE_CHANNEL else (B, H, nG), dtype=f32, device=device)
         self.O = torch.zeros((B, H, N, D), dtype=f16, device=device)
         self.ws = torch.empty(rotattn_workspace_bytes(p, 0), dtype=u8, device=device)
         self.Q16 = self.K16 = self.O16 = self.ws16 = None
@@ -144,23 +156,27 @@ class Buffers:
             self.Q16 = torch.empty((B, H, N, D), dtype=f16, device=device)
             self.K16 = torch.empty_like(self.Q16)
             self.O16 = torch.zeros_like(self.Q16)
-            self.ws16 = torch.empty(rotattn_workspace_bytes(p, 1), dtype=u8, device=device)
+            self.ws16 = torch.empty(rotattn_workspace_bytes(p, 2), dtype=u8, device=device)
 
 
-def params_for(w, rot_mode=ROT_HALF, p_mode=P_ASYM15, p_norm=NORM_ROWBLOCK, H=None):
-    return make_params(w.B, w.H if H is None else H, w.N, w.D, w.grid, w.pairs, 10000.0, rot_mode, p_mode, p_norm)
+def params_for(w, rot_mode=ROT_HALF, p_mode=P_ASYM15, p_norm=NORM_ROWBLOCK, H=None, qk_group=1,
+               v_scale=VSCALE_CHANNEL, smooth=0):
+    return make_params(w.B, w.H if H is None else H, w.N, w.D, w.grid, w.pairs, 10000.0, rot_mode, p_mode, p_norm,
+                       qk_group=qk_group, v_scale=v_scale, smooth=smooth)
 
 
 def run_int4(w, q, k, v, rot_mode=ROT_HALF, p_mode=P_ASYM15, p_norm=NORM_ROWBLOCK, want_fp16=False,
-             coef=None, rot=None, use_ws=True):
+             coef=None, rot=None, use_ws=True, qk_group=1, v_scale=VSCALE_CHANNEL, smooth=0):
     """Whole hot path on numpy fp16 inputs [B,H',N,D]; returns a dict of device tensors."""
-    p = params_for(w, rot_mode, p_mode, p_norm, H=q.shape[1])
+    p = params_for(w, rot_mode, p_mode, p_norm, H=q.shape[1], qk_group=qk_group, v_scale=v_scale, smooth=smooth)
     tab = rotattn_build_tables(p, rot) if coef is None else np.ascontiguousarray(coef, dtype=np.float32)
     coef_dev = torch.from_numpy(tab).cuda()
     rot_dev = None if rot is None else torch.from_numpy(np.ascontiguousarray(rot, dtype=np.float32)).cuda()
     Q, K, V = (torch.from_numpy(x).cuda() for x in (q, k, v))
     b = Buffers(p, want_fp16)
     ws = b.ws if use_ws else None
+    if smooth:
+        rotattn_smooth_stats(p, coef_dev, rot_dev, Q, K, V, b.ws)
     rotattn_prepare_qk(p, coef_dev, rot_dev, Q, K, b.Q4, b.Qs, b.K4, b.Ks, b.Q16, b.K16, ws)
     rotattn_quant_v(p, V, b.V4, b.Vs, ws)
     rotattn_fwd_int4(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, b.O, b.ws, (WS_HAS_QK | WS_HAS_V) if use_ws else 0)

@@ -9,22 +9,23 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, 'librotattn.so')
 
-ROT_NONE, ROT_INTERLEAVED, ROT_HALF = 0, 1, 2
+ROT_NONE, ROT_INTERLEAVED, ROT_HALF, ROT_FULL = 0, 1, 2, 3
 P_ASYM15, P_SYM7 = 0, 1
 NORM_ROWBLOCK, NORM_RUNNING = 0, 1
 WS_HAS_QK, WS_HAS_V = 1, 2
+VSCALE_CHANNEL, VSCALE_GROUP = 0, 1
 
 
 class RotattnParams(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ('B', 'H', 'N', 'D', 'grid_t', 'grid_h', 'grid_w',
                                          'pairs_t', 'pairs_h', 'pairs_w')] + \
                [('rope_base', C.c_float)] + \
-               [(n, C.c_int32) for n in ('rot_mode', 'p_mode', 'p_norm', 'qk_group', 'v_group', 'kv_block')]
+               [(n, C.c_int32) for n in ('rot_mode', 'p_mode', 'p_norm', 'qk_group', 'v_group', 'kv_block', 'v_scale', 'smooth')]
 
 
 class RotattnPolicy(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ('n_steps', 'n_blocks', 'first_steps', 'last_steps',
-                                         'first_blocks', 'last_blocks')] + \
+                                         'first_blocks', 'last_blocks', 'n_heads')] + \
                [('fp16_head_mask', C.POINTER(C.c_uint8))]
 
 
@@ -47,7 +48,9 @@ EXPORTS = {
     'rotattn_prepare_qk': (C.c_int, [_P, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
     'rotattn_quant_v': (C.c_int, [_P, _vp, _vp, _vp, _vp, _sz, _vp]),
     'rotattn_fwd_int4': (C.c_int, [_P, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _i32, _vp, _sz, _i32, _vp]),
-    'rotattn_fwd_int4_debug': (C.c_int, [_P, _vp, _vp, _vp, _vp, _vp, _vp, _i32, _i32, _vp, _vp, _vp, _vp, _sz, _i32, _vp]),
+    'rotattn_smooth_stats': (C.c_int, [_P, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
+    'rotattn_smooth_read': (C.c_int, [_P, _vp, _sz, _vp, _vp, _vp]),
+    'rotattn_fwd_int4_debug': (C.c_int, [_P, _vp, _vp, _vp, _vp, _vp, _vp, _i32, _i32, _vp, _vp, _vp, _vp, _vp, _sz, _i32, _vp]),
     'rotattn_fwd_fp16': (C.c_int, [_P, _vp, _vp, _vp, _vp, _vp, _i32, _vp, _sz, _vp]),
     'rotattn_probe_gemm8': (C.c_int, [_i32, _i32, _i32, _vp, _vp, _vp, _i32, _vp]),
 }
@@ -69,6 +72,7 @@ def check(status: int, what: str):
 
 
 def make_params(B, H, N, D, grid, pairs, rope_base=10000.0, rot_mode=ROT_HALF, p_mode=P_ASYM15,
-                p_norm=NORM_ROWBLOCK, qk_group=1, v_group=128, kv_block=128) -> RotattnParams:
+                p_norm=NORM_ROWBLOCK, qk_group=1, v_group=128, kv_block=128, v_scale=VSCALE_CHANNEL,
+                smooth=0) -> RotattnParams:
     return RotattnParams(B, H, N, D, grid[0], grid[1], grid[2], pairs[0], pairs[1], pairs[2], rope_base,
-                         rot_mode, p_mode, p_norm, qk_group, v_group, kv_block)
+                         rot_mode, p_mode, p_norm, qk_group, v_group, kv_block, v_scale, smooth)

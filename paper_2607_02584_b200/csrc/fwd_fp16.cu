@@ -122,7 +122,7 @@ fwd_fp16_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       for (int j = 0; j < nblk; ++j) {
         const int s = j % F_STAGES;
         const uint32_t ph = (j / F_STAGES) & 1;
-        mbar_wait_relaxed(&k_empty[s], ph ^ 1);
+        mbar_wait(&k_empty[s], ph ^ 1);
         if (elect_one()) {
           mbar_arrive_expect_tx(&k_full[s], L::K_BYTES);
 #pragma unroll
@@ -130,7 +130,7 @@ fwd_fp16_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tma_load_3d(sK + s * L::K_BYTES + pn * 16384, &tmK, &k_full[s], pn * 64, j * kTile, bh);
         }
         __syncwarp();
-        mbar_wait_relaxed(&v_empty[s], ph ^ 1);
+        mbar_wait(&v_empty[s], ph ^ 1);
         if (elect_one()) {
           mbar_arrive_expect_tx(&v_full[s], L::V_BYTES);
 #pragma unroll

@@ -1,499 +1,28 @@
-// rotattn_fwd_int4 (steps a4-a9): INT4 FlashAttention forward on tcgen05 (kind::f8f6f4 on integer-exact E4M3 code
-// bytes, see fwd_int4.cuh), row-block P normaliser.
-//
-// One CTA = one 128-row query tile of one (b,h); 28 warps, warp-specialised:
-//   warps 0-7     softmax group 0: even KV blocks; warps 0-3 own keys [0,64) of the block, warps 4-7 keys [64,128)
-//   warps 8-15    softmax group 1: odd KV blocks, same split  (two threads per query row and block)
-//   warps 16-23   drain: 2 threads per query row (D/2 channels each): online-softmax bookkeeping (m, l, alpha, beta),
-//                 P~V block -> fp32 O registers, epilogue O/l
-//   warp 24       TMEM allocator, then scale loader (Ks[j] * 2^18 log2e/sqrt(D) and Vs[g][:] -> shared rings)
-//   warp 25       TMA producer  : Q tile once, K tiles (4-stage ring) and V^T tiles (3-stage ring)
-//   warp 26       MMA issuer 2  : P~V (P codes x V codes, both from shared memory, TMEM accumulators)
-//   warp 27       MMA issuer 1  : S = Q K^T (codes x codes, exact, TMEM)
-// With the row-block normaliser (reading 13) the codes of block j depend only on block j, so the two softmax
-// groups work on different blocks concurrently and the running max lives in the drain threads.  Each softmax thread
-// makes two passes over its half row of S in tensor memory in 16-column chunks: pass 1 scales by the key scales, writes
-// t back over S and takes the block row max (exchanged with the partner thread through shared memory); pass 2 reads t:
-// exp2 / row sum / codes.
-// TMEM (512 columns): S[2] at 0/128 and four half-width (D/2 channels) P~V accumulators of 64 columns at 256 (block
-// parity x channel half), so that the P~V MMAs run a block ahead of the drain instead of alternating with it.  The u8 P
-// codes go to four shared-memory tiles (128-byte swizzle, A operand from shared memory), so an S buffer is released as
-// soon as pass 2 has read it (S(j+2) is issued before P~V(j), hiding the MMA latency).
-// The per-block drain is forced by the method: beta (row, block) and Vs (channel, block) change every KV block
-// (PAPER.md:L157 online softmax, L190 per-group V scales), so P~V cannot accumulate across blocks in tensor memory.
+// rotattn_fwd_int4 / rotattn_fwd_int4_debug: host side of the INT4 attention kernels (argument checks, workspace
+// copies, tensor maps, variant dispatch).  The kernels are in fwd_int4_kernel.cuh (ROWBLOCK normaliser) and
+// fwd_int4_sync.cu (RUNNING normaliser).
 #include <cmath>
 #include <cstdio>
-#include <type_traits>
 #include "fwd_int4.cuh"
-
-namespace rotattn {
-
-#if defined(ROTATTN_SDONE_RELAXED)
-#define mbar_wait_sdone mbar_wait_relaxed
-#elif defined(ROTATTN_SDONE_SPIN)
-#define mbar_wait_sdone mbar_wait_spin
-#else
-#define mbar_wait_sdone mbar_wait
-#endif
-#if defined(ROTATTN_SEMPTY_SPIN)
-#define mbar_wait_sempty mbar_wait_spin
-#else
-#define mbar_wait_sempty mbar_wait
-#endif
-
-constexpr int kFwdThreads = 896;
-// Warp roles.  Within an SM sub-partition the scheduler favours the highest warp id among the eligible warps, so the
-// latency-critical single-thread roles (MMA issue, TMA) get the highest ids and the throughput roles the lowest.
-constexpr int kWarpScale = 24, kWarpTma = 25, kWarpMmaPV = 26, kWarpMmaS = 27;
-constexpr int K_STAGES = 4;
-constexpr int V_STAGES = 3;
-constexpr int P_SLOTS = 4;       // P-code tiles in shared memory (A operand of the P~V MMA)
-constexpr int PV_BUFS = 4;       // half-width (D/2 channel) P~V accumulators in rotation: buffer 2 * (j & 1) + h
-constexpr int AB_RING = 8;
-constexpr int KS_RING = 4;
-constexpr int VS_RING = 4;
-static_assert(K_STAGES == 4 && P_SLOTS == 4 && PV_BUFS == 4 && V_STAGES <= P_SLOTS && KS_RING == VS_RING, "ring sizes are tied together by the shared completion barriers");
-
-template <int D>
-struct SmemInt4 {
-  static constexpr int Q_BYTES = 128 * 128;
-  static constexpr int K_BYTES = 128 * 128;
-  static constexpr int V_BYTES = D * 128;
-  static constexpr int OFF_Q = 0;
-  static constexpr int OFF_K = OFF_Q + Q_BYTES;
-  static constexpr int OFF_V = OFF_K + K_STAGES * K_BYTES;
-  static constexpr int P_BYTES = 128 * 128;                           // u8 codes [128 query rows][128 keys], 128-byte swizzle
-  static constexpr int OFF_P = OFF_V + V_STAGES * V_BYTES;
-  static constexpr int OFF_KS = OFF_P + P_SLOTS * P_BYTES;            // float [KS_RING][128]
-  static constexpr int OFF_VS = OFF_KS + KS_RING * 128 * 4;           // float [VS_RING][D]
-  static constexpr int OFF_AB = OFF_VS + VS_RING * D * 4;             // float [AB_RING][3][128]: block max, half-row sums of the two key halves
-  static constexpr int OFF_MX = OFF_AB + AB_RING * 3 * 128 * 4;       // float [2 groups][2 parities][2 halves][128]
-  static constexpr int OFF_BAR = OFF_MX + 2 * 2 * 2 * 128 * 4;        // mbarriers
-  static constexpr int NBAR = 1 + 2 * K_STAGES + V_STAGES + 2 + 2 * P_SLOTS + 2 * PV_BUFS + AB_RING + 2 * KS_RING + 2 * VS_RING;
-  static constexpr int OFF_TMEM = OFF_BAR + NBAR * 8;
-  static constexpr int TOTAL = OFF_TMEM + 16;
-};
-
-// ---- per-chunk element-wise work of the softmax threads (16 S columns of one query row) -------------------------
-// Pass 1: t = S * (Ks_j * 2^18 log2e/sqrt(D)) (the query scale Qs_i > 0 is applied after the max); keys >= N are masked
-// to -inf.  t overwrites S in tensor memory so that pass 2 needs neither the key scales nor the mask.
-template <bool MASK>
-__device__ __forceinline__ void chunk_scale_max(const uint32_t (&v)[16], const float2* ks2, int nvalid_rel, uint32_t (&t)[16],
-                                                float& mx0, float& mx1) {
-#pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    float2 t2 = fmul2(make_float2(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1])), ks2[i]);
-    if (MASK) {
-      if (2 * i >= nvalid_rel) t2.x = -INFINITY;
-      if (2 * i + 1 >= nvalid_rel) t2.y = -INFINITY;
-    }
-    if (i & 1) mx1 = fmax3(mx1, t2.x, t2.y); else mx0 = fmax3(mx0, t2.x, t2.y);
-    t[2 * i] = __float_as_uint(t2.x);
-    t[2 * i + 1] = __float_as_uint(t2.y);
-  }
-}
-
-// Pass 2: LEVELS * P^ = exp2(t * Qs_i - mt + log2(LEVELS)); codes u = rne(LEVELS * P^) taken from the low byte of
-// (LEVELS * P^) + 1.5 * 2^23 (Eq.12 L166-168 with the fixed scale 15 / Eq.11 L161 with 7); four codes per TMEM column.
-__device__ __forceinline__ void chunk_exp(const uint32_t (&t)[16], float2 qs2, float2 nref2, float2& ls0, float2& ls1, uint32_t (&pw)[4]) {
-  const float2 magic2 = make_float2(12582912.f, 12582912.f);
-#pragma unroll
-  for (int g = 0; g < 4; ++g) {
-    const float2 e0 = ffma2(make_float2(__uint_as_float(t[4 * g]), __uint_as_float(t[4 * g + 1])), qs2, nref2);
-    const float2 e1 = ffma2(make_float2(__uint_as_float(t[4 * g + 2]), __uint_as_float(t[4 * g + 3])), qs2, nref2);
-    const float2 p0 = make_float2(ex2_approx(e0.x), ex2_approx(e0.y));
-    const float2 p1 = make_float2(ex2_approx(e1.x), ex2_approx(e1.y));
-    ls0 = fadd2(ls0, p0);
-    ls1 = fadd2(ls1, p1);
-    const float2 f0 = fadd2(p0, magic2), f1 = fadd2(p1, magic2);
-    const uint32_t lo = __byte_perm(__float_as_uint(f0.x), __float_as_uint(f0.y), 0x0040);
-    const uint32_t hi = __byte_perm(__float_as_uint(f1.x), __float_as_uint(f1.y), 0x0040);
-    pw[g] = __byte_perm(lo, hi, 0x5410);
-  }
-}
-
-template <int D, int P_MODE, bool DEBUG>
-__global__ void __launch_bounds__(kFwdThreads, 1)
-fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
-                const __grid_constant__ CUtensorMap tmV, const FwdInt4Args a) {
-  using L = SmemInt4<D>;
-  extern __shared__ __align__(1024) uint8_t smem[];      // no static shared memory in this kernel: base is 1024-aligned
-  uint8_t* sQ = smem + L::OFF_Q;
-  uint8_t* sK = smem + L::OFF_K;
-  uint8_t* sV = smem + L::OFF_V;
-  uint8_t* sP = smem + L::OFF_P;
-  float* sKs = (float*)(smem + L::OFF_KS);
-  float* sVs = (float*)(smem + L::OFF_VS);
-  float* sAB = (float*)(smem + L::OFF_AB);
-  float* sMx = (float*)(smem + L::OFF_MX);
-  uint64_t* bars = (uint64_t*)(smem + L::OFF_BAR);
-  uint64_t* q_full = bars;
-  uint64_t* k_full = q_full + 1;              // [K_STAGES] TMA -> MMA
-  uint64_t* v_full = k_full + K_STAGES;       // [V_STAGES] TMA -> MMA
-  uint64_t* s_done = v_full + V_STAGES;       // [K_STAGES] S(m) complete: -> softmax group m & 1 (S ready), -> TMA (K stage free)
-  uint64_t* s_empty = s_done + K_STAGES;      // [2] softmax group -> MMA (count 256): S buffer has been read
-  uint64_t* p_full = s_empty + 2;             // [P_SLOTS] softmax group -> MMA (count 256)
-  uint64_t* pv_done = p_full + P_SLOTS;       // [P_SLOTS] both halves of P~V(j) complete: -> softmax (P slot free), TMA (V stage free)
-  uint64_t* pvh_done = pv_done + P_SLOTS;    // [PV_BUFS] half k = 2j+h of P~V complete -> drain warps of channel half h
-  uint64_t* pvh_empty = pvh_done + PV_BUFS;   // [PV_BUFS] drain -> MMA (count 128): half buffer is in registers
-  uint64_t* ab_full = pvh_empty + PV_BUFS;    // [AB_RING] softmax -> drain (count 256)
-  uint64_t* ks_full = ab_full + AB_RING;      // [KS_RING] loader -> softmax (count 32)
-  uint64_t* ks_empty = ks_full + KS_RING;     // [KS_RING] softmax -> loader (count 256)
-  uint64_t* vs_full = ks_empty + KS_RING;     // [VS_RING] loader -> drain (count 32)
-  uint64_t* vs_empty = vs_full + VS_RING;     // [VS_RING] drain -> loader (count 256)
-  uint32_t* tmem_slot = (uint32_t*)(smem + L::OFF_TMEM);
-
-  const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);   // warp-uniform (kept in a uniform register)
-  const int lane = threadIdx.x & 31;
-  const int qtile = DEBUG ? a.dbg_qtile : blockIdx.x;
-  const int bh = DEBUG ? a.dbg_bh : (a.head_sel ? a.head_sel[blockIdx.y] : (int)blockIdx.y);
-  const int q0 = qtile * kTile;
-  const int nblk = a.nblk;
-
-  if (threadIdx.x == 0) {
-    if (smem_u32(smem) & 1023u) __trap();     // SWIZZLE_128B operand tiles need 1024-byte alignment
-    mbar_init(q_full, 1);
-    for (int i = 0; i < K_STAGES; ++i) { mbar_init(&k_full[i], 1); mbar_init(&s_done[i], 1); }
-    for (int i = 0; i < V_STAGES; ++i) mbar_init(&v_full[i], 1);
-    for (int i = 0; i < 2; ++i) mbar_init(&s_empty[i], 256);
-    for (int i = 0; i < P_SLOTS; ++i) mbar_init(&p_full[i], 256);
-    for (int i = 0; i < P_SLOTS; ++i) mbar_init(&pv_done[i], 1);
-    for (int i = 0; i < PV_BUFS; ++i) { mbar_init(&pvh_done[i], 1); mbar_init(&pvh_empty[i], 128); }
-    for (int i = 0; i < AB_RING; ++i) mbar_init(&ab_full[i], 256);
-    for (int i = 0; i < KS_RING; ++i) { mbar_init(&ks_full[i], 32); mbar_init(&ks_empty[i], 256); }
-    for (int i = 0; i < VS_RING; ++i) { mbar_init(&vs_full[i], 32); mbar_init(&vs_empty[i], 256); }
-    fence_mbar_init();
-  }
-  if (warp == kWarpScale) tmem_alloc(tmem_slot, 512);
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem_base = *tmem_slot;
-  constexpr uint32_t TM_S = 0, TM_PV = 256;                 // S[2] x 128 | PV half buffers [4] x 64
-
-  // register pool of the CTA = 896 x 72; after redistribution 128 x 24 + 512 x 72 + 256 x 96 = 64512 (exactly the pool)
-  if (warp >= 24) {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
-    // The single-thread roles keep warp-uniform control flow (every lane waits; one elected lane issues), so that the
-    // TMA / MMA operands stay in uniform registers.
-    if (warp == kWarpTma) {
-      // ---------------------------------------------------------------- TMA producer
-      if (elect_one()) {
-        tma_prefetch_desc(&tmQ); tma_prefetch_desc(&tmK); tma_prefetch_desc(&tmV);
-        mbar_arrive_expect_tx(q_full, L::Q_BYTES);
-        tma_load_3d(sQ, &tmQ, q_full, 0, q0, bh);
-      }
-      __syncwarp();
-      for (int i = 0; i < nblk + 2; ++i) {
-        const int m = i, j = i - 2;                                      // K runs two blocks ahead of V
-        if (m < nblk) {
-          const int s = m % K_STAGES;
-          mbar_wait_relaxed(&s_done[s], ((m / K_STAGES) & 1) ^ 1);               // S(m-4) has consumed this K stage
-          if (elect_one()) {
-            mbar_arrive_expect_tx(&k_full[s], L::K_BYTES);
-            tma_load_3d(sK + s * L::K_BYTES, &tmK, &k_full[s], 0, m * kTile, bh);
-          }
-          __syncwarp();
-        }
-        if (j >= 0) {
-          const int s = j % V_STAGES;
-          if (j >= V_STAGES) mbar_wait_relaxed(&pv_done[(j - V_STAGES) % P_SLOTS], ((j - V_STAGES) / P_SLOTS) & 1);   // P~V(j-3) has consumed this V stage
-          if (elect_one()) {
-            mbar_arrive_expect_tx(&v_full[s], L::V_BYTES);
-            tma_load_3d(sV + s * L::V_BYTES, &tmV, &v_full[s], j * kTile, 0, bh);
-          }
-          __syncwarp();
-        }
-      }
-    } else if (warp == kWarpMmaS) {
-      // ---------------------------------------------------------------- MMA issuer 1: S(m) = Q K(m)^T -> buffer m & 1
-      constexpr uint32_t idesc_s = umma_idesc(1, 0, 0, 128, 128);        // f32 <- e4m3 x e4m3 (integer codes * 2^-9)
-      constexpr int KSTEPS_S = D / 32;                                   // D=64 rows are zero-padded to 128 B
-      const uint64_t qd = umma_desc_k128(smem_u32(sQ));
-      mbar_wait(q_full, 0);
-      for (int m = 0; m < nblk; ++m) {
-        const int st = m % K_STAGES, b = m & 1;
-        ROTATTN_STAMP(m, 4);
-        mbar_wait_relaxed(&k_full[st], (m / K_STAGES) & 1);
-        ROTATTN_STAMP(m, 5);
-        if (m >= 2) mbar_wait_sempty(&s_empty[b], ((m >> 1) - 1) & 1);          // softmax has read S(m-2) out of this buffer
-        tc_fence_after();
-        ROTATTN_STAMP(m, 6);
-        if (elect_one()) {
-          const uint64_t kd = umma_desc_k128(smem_u32(sK + st * L::K_BYTES));
-#pragma unroll
-          for (int k = 0; k < KSTEPS_S; ++k)
-            mma_ss<MmaKind::F8F6F4>(tmem_base + TM_S + b * 128, qd + 2 * k, kd + 2 * k, idesc_s, k != 0);
-          tc_commit(&s_done[st]);                                        // -> softmax group (S ready) and TMA (K stage free)
-        }
-        __syncwarp();
-        ROTATTN_STAMP(m, 0);
-      }
-    } else if (warp == kWarpMmaPV) {
-      // ---------------------------------------------------------------- MMA issuer 2: PV = P~(j) V(j)
-      constexpr uint32_t idesc_pv = umma_idesc(1, 0, 0, 128, D / 2);
-      for (int j = 0; j < nblk; ++j) {
-        const int slot = j % P_SLOTS, vst = j % V_STAGES;
-        mbar_wait_relaxed(&v_full[vst], (j / V_STAGES) & 1);
-        mbar_wait_relaxed(&p_full[slot], (j / P_SLOTS) & 1);
-        ROTATTN_STAMP(j, 1);
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          const int buf = 2 * (j & 1) + h;
-          mbar_wait_relaxed(&pvh_empty[buf], ((j >> 1) & 1) ^ 1);                // drain has read half (j-2, h) out of this buffer
-          tc_fence_after();
-          if (h == 0) ROTATTN_STAMP(j, 3);
-          if (elect_one()) {
-            // V^T tile: channel half h starts D/2 rows (= D/2 * 128 B, whole 1024-byte swizzle atoms) into the tile
-            const uint64_t pd = umma_desc_k128(smem_u32(sP + slot * L::P_BYTES));
-            const uint64_t vd = umma_desc_k128(smem_u32(sV + vst * L::V_BYTES + h * (D / 2) * 128));
-#pragma unroll
-            for (int k = 0; k < 4; ++k)
-              mma_ss<MmaKind::F8F6F4>(tmem_base + TM_PV + buf * 64, pd + 2 * k, vd + 2 * k, idesc_pv, k != 0);
-            tc_commit(&pvh_done[buf]);                                   // -> drain warps of this channel half
-            if (h == 1) tc_commit(&pv_done[slot]);                        // -> softmax (P slot free), TMA (V stage free)
-          }
-          __syncwarp();
-        }
-        ROTATTN_STAMP(j, 9);
-      }
-    } else {
-      // ---------------------------------------------------------------- scale loader: Ks_j * 2^18 log2e/sqrt(D), Vs[g][:]
-      const float* ksrc = a.Ks + (size_t)bh * a.N;
-      const float* vsrc = a.Vs + (size_t)bh * nblk * D;
-      for (int j = 0; j < nblk; ++j) {
-        const int s = j % KS_RING;
-        float kv[4], vv[D / 32];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          const int kj = j * kTile + i * 32 + lane;
-          kv[i] = (kj < a.N) ? ksrc[kj] * a.scale_log2 : 0.f;
-        }
-#pragma unroll
-        for (int i = 0; i < D / 32; ++i) vv[i] = vsrc[(size_t)j * D + i * 32 + lane];
-        mbar_wait_relaxed(&ks_empty[s], ((j / KS_RING) & 1) ^ 1);
-#pragma unroll
-        for (int i = 0; i < 4; ++i) sKs[s * 128 + i * 32 + lane] = kv[i];
-        mbar_arrive(&ks_full[s]);
-        mbar_wait_relaxed(&vs_empty[s], ((j / VS_RING) & 1) ^ 1);
-#pragma unroll
-        for (int i = 0; i < D / 32; ++i) sVs[s * D + i * 32 + lane] = vv[i];
-        mbar_arrive(&vs_full[s]);
-      }
-    }
-  } else if (warp < 16) {
-    // ------------------------------------------------------------------ softmax groups: 0 = even blocks, 1 = odd blocks
-    constexpr float LOG2_LEVELS = P_MODE == ROTATTN_P_ASYM15 ? 3.9068905956085187f : 2.8073549220576042f;
-    const int g = warp >> 3;                         // group index = S buffer index
-    const int h = (warp >> 2) & 1;                   // which 64 keys of the block
-    const int r = (warp & 3) * 32 + lane;
-    const int row = q0 + r;
-    const int cb = 64 * h;
-    const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
-    // qs >= 1e-30 keeps (-inf) * qs well defined for masked keys; an all-zero query row still gives s == 0 everywhere
-    const float qs = (row < a.N) ? fmaxf(a.Qs[(size_t)bh * a.N + row], 1e-30f) : 1e-30f;
-    const float2 qs2 = make_float2(qs, qs);
-    const uint32_t s_addr = tmem_base + lane_off + TM_S + g * 128 + cb;
-    const int pair_bar = 1 + 4 * g + (warp & 3);     // named barrier of the two warps that share these 32 rows
-    for (int j = g; j < nblk; j += 2) {
-      const int n = j >> 1;
-      const int ring = j % KS_RING, slot = j % P_SLOTS, abslot = j % AB_RING;
-      const float2* ks2 = reinterpret_cast<const float2*>(sKs + ring * 128 + cb);
-      const int nvalid = min(kTile, a.N - j * kTile) - cb;   // valid keys of this half; < 64 only on the ragged last block
-      const bool ragged = nvalid < 64;
-      mbar_wait(&ks_full[ring], (j / KS_RING) & 1);
-      mbar_wait_sdone(&s_done[j % K_STAGES], (j / K_STAGES) & 1);
-      tc_fence_after();
-      ROTATTN_STAMP(j, 0);
-      uint32_t va[16], vb[16], tt[16];
-      // ---- pass 1: t = S * ks (written back over S), block row max over this half
-      float mx0 = -INFINITY, mx1 = -INFINITY;
-      tmem_ld16(s_addr, va);
-      auto pass1 = [&](auto masked) {                    // one branch per block on the ragged case, not one per chunk
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-          tmem_wait_ld();
-          uint32_t(&cur)[16] = (c & 1) ? vb : va;
-          uint32_t(&nxt)[16] = (c & 1) ? va : vb;
-          if (c < 3) tmem_ld16(s_addr + (c + 1) * 16, nxt);
-          if (DEBUG) {
-#pragma unroll
-            for (int i = 0; i < 16; ++i)
-              a.S_dump[(size_t)r * a.npad + j * kTile + cb + c * 16 + i] = (int32_t)(__uint_as_float(cur[i]) * kAccScale);
-          }
-#if defined(ROTATTN_ABL) && (ROTATTN_ABL == 3 || ROTATTN_ABL == 6)      // development ablation: no pass-1 arithmetic / write-back
-          mx0 = fmaxf(mx0, __uint_as_float(cur[0]));
-#else
-          chunk_scale_max<decltype(masked)::value>(cur, ks2 + c * 8, nvalid - c * 16, tt, mx0, mx1);
-          tmem_st16(s_addr + c * 16, tt);
-#endif
-        }
-      };
-      if (ragged) pass1(std::true_type{}); else pass1(std::false_type{});
-      ROTATTN_STAMP(j, 1);
-      float tmax = fmaxf(mx0, mx1);
-      float* mxbuf = sMx + ((g * 2 + (n & 1)) * 2) * 128;
-      mxbuf[h * 128 + r] = tmax;
-      mbar_arrive(&ks_empty[ring]);
-      tmem_wait_st();
-      tmem_ld16(s_addr, va);                             // chunk 0 of t, in flight across the max exchange
-      bar_sync(pair_bar, 64);
-      tmax = fmaxf(tmax, mxbuf[(h ^ 1) * 128 + r]);
-      const float mt = qs * tmax;                        // block row max of s * log2e
-      const float nref = LOG2_LEVELS - mt;
-      const float2 nref2 = make_float2(nref, nref);
-      mbar_wait(&pv_done[slot], ((j / P_SLOTS) & 1) ^ 1);            // P~V(j-4) has consumed this P slot
-      ROTATTN_STAMP(j, 2);
-      // ---- pass 2: LEVELS * P^, row sum, codes -> u8 P tile slot
-      float2 ls0 = make_float2(0.f, 0.f), ls1 = make_float2(0.f, 0.f);
-      uint8_t* p_row = sP + slot * L::P_BYTES + r * 128;             // 16-byte chunk q of row r lives at chunk q ^ (r & 7)
-#pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        tmem_wait_ld();
-        uint32_t(&cur)[16] = (c & 1) ? vb : va;
-        uint32_t(&nxt)[16] = (c & 1) ? va : vb;
-        if (c < 3) tmem_ld16(s_addr + (c + 1) * 16, nxt);
-        else { tc_fence_before(); mbar_arrive(&s_empty[g]); }          // this thread is done with the S buffer
-        uint32_t pw[4];
-#if defined(ROTATTN_ABL) && (ROTATTN_ABL == 4 || ROTATTN_ABL == 6)   // development ablation: no pass-2 arithmetic
-        pw[0] = cur[0]; pw[1] = cur[1]; pw[2] = cur[2]; pw[3] = cur[3];
-#else
-        chunk_exp(cur, qs2, nref2, ls0, ls1, pw);
-#endif
-        if (DEBUG) {
-#pragma unroll
-          for (int q = 0; q < 4; ++q) *reinterpret_cast<uint32_t*>(a.P_dump + (size_t)r * a.npad + j * kTile + cb + c * 16 + q * 4) = pw[q];
-        }
-        *reinterpret_cast<uint4*>(p_row + (((4 * h + c) ^ (r & 7)) << 4)) = make_uint4(pw[0], pw[1], pw[2], pw[3]);
-      }
-      if (h == 0) sAB[(abslot * 3) * 128 + r] = mt;
-      sAB[(abslot * 3 + 1 + h) * 128 + r] = (ls0.x + ls0.y) + (ls1.x + ls1.y);
-      ROTATTN_STAMP(j, 3);
-      fence_proxy_async_smem();                          // P codes (generic-proxy stores) -> visible to the MMA (async proxy)
-      mbar_arrive(&p_full[slot]);
-      ROTATTN_STAMP(j, 4);
-      mbar_arrive(&ab_full[abslot]);
-    }
-  } else {
-    // ------------------------------------------------------------------ drain: 2 threads per query row of O
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 96;");
-    constexpr int DH = D / 2;                      // channels per thread
-    const int h = (warp >> 2) & 1, r = (warp & 3) * 32 + lane;
-    const int row = q0 + r;
-    const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
-    float2 o2[DH / 2];
-#pragma unroll
-    for (int d = 0; d < DH / 2; ++d) o2[d] = make_float2(0.f, 0.f);
-    // Online softmax bookkeeping (L157) with a lazily updated reference max: O and l are kept relative to m_ref, which
-    // only moves when a block max exceeds it by more than 2^8 (fp32 has the headroom), so the common path is
-    // O += beta * pv * Vs with beta = exp2(mt - m_ref) and no rescale of the 64 accumulators.
-    constexpr float kLazy = 8.f;
-    float m_ref = -INFINITY, l_run = 0.f;
-    for (int j = 0; j < nblk; ++j) {
-      const int abslot = j % AB_RING;
-      ROTATTN_STAMP(j, 0);
-      mbar_wait_relaxed(&ab_full[abslot], (j / AB_RING) & 1);
-      ROTATTN_STAMP(j, 1);
-      const float mt = sAB[(abslot * 3) * 128 + r];
-      const float bsum = sAB[(abslot * 3 + 1) * 128 + r] + sAB[(abslot * 3 + 2) * 128 + r];
-      const int vring = j % VS_RING;
-      const int buf = 2 * (j & 1) + h;
-      const uint32_t pv_addr = tmem_base + lane_off + TM_PV + buf * 64;
-      mbar_wait_relaxed(&vs_full[vring], (j / VS_RING) & 1);
-      mbar_wait_relaxed(&pvh_done[buf], (j >> 1) & 1);
-      tc_fence_after();
-      ROTATTN_STAMP(j, 2);
-      uint32_t va[16], vb[16];
-      tmem_ld16(pv_addr, va);                                          // in flight across the bookkeeping below
-      if (__any_sync(0xffffffffu, mt > m_ref + kLazy)) {               // rare after the first blocks (warp-uniform branch)
-        const float m_new = (mt > m_ref + kLazy) ? mt : m_ref;
-        const float alpha = ex2_approx(m_ref - m_new);                 // first block: exp2(-inf) = 0; unchanged rows: 1
-        const float2 a2 = make_float2(alpha, alpha);
-#pragma unroll
-        for (int d = 0; d < DH / 2; ++d) o2[d] = fmul2(o2[d], a2);
-        l_run *= alpha;
-        m_ref = m_new;
-      }
-      const float beta = ex2_approx(mt - m_ref);                       // <= 2^8
-      l_run = fmaf(beta, bsum, l_run);                                 // in units of LEVELS (cancels in O/l)
-      const float cf = beta * kAccScale;                               // undoes the 2^-18 of the E4M3 code products
-      const float2 c2 = make_float2(cf, cf);
-      const float2* vsb2 = reinterpret_cast<const float2*>(sVs + vring * D + h * DH);
-#pragma unroll
-      for (int cc = 0; cc < DH / 16; ++cc) {
-        tmem_wait_ld();
-        uint32_t(&cur)[16] = (cc & 1) ? vb : va;
-        uint32_t(&nxt)[16] = (cc & 1) ? va : vb;
-        ROTATTN_STAMP(j, 4 + cc);
-        if (cc + 1 < DH / 16) tmem_ld16(pv_addr + (cc + 1) * 16, nxt);
-        else { tc_fence_before(); mbar_arrive(&pvh_empty[buf]); }      // this half-width accumulator is in registers now
-#if !(defined(ROTATTN_ABL) && (ROTATTN_ABL == 2 || ROTATTN_ABL == 6))
-#pragma unroll
-        for (int d = 0; d < 8; ++d) {
-          const float2 y = fmul2(make_float2(__uint_as_float(cur[2 * d]), __uint_as_float(cur[2 * d + 1])), vsb2[cc * 8 + d]);
-          o2[cc * 8 + d] = ffma2(y, c2, o2[cc * 8 + d]);               // O += beta * pv * Vs[g][d]
-        }
-#else
-        o2[cc].x += __uint_as_float(cur[0]);
-#endif
-      }
-      mbar_arrive(&vs_empty[vring]);
-      ROTATTN_STAMP(j, 3);
-    }
-    const float inv_l = 1.f / l_run;
-    if (row < a.N) {
-      __half* dst = (DEBUG ? a.O + (size_t)r * D : a.O + ((size_t)bh * a.N + row) * D) + h * DH;
-#pragma unroll
-      for (int d = 0; d < DH; d += 8) {
-        __half2 hh[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) hh[i] = __floats2half2_rn(o2[d / 2 + i].x * inv_l, o2[d / 2 + i].y * inv_l);
-        *reinterpret_cast<uint4*>(dst + d) = *reinterpret_cast<uint4*>(hh);
-      }
-    }
-  }
-  tc_fence_before();
-  __syncthreads();
-  if (warp == kWarpScale) tmem_dealloc(tmem_base, 512);
-}
-
-}  // namespace rotattn
 
 using namespace rotattn;
 
-#ifdef ROTATTN_TRACE
-static long long* g_rotattn_trace = nullptr;
-extern "C" void rotattn_set_trace(long long* p) { g_rotattn_trace = p; }
-#endif
-
 namespace {
-
-template <int D, bool DEBUG>
-int launch_variant(const rotattn_params& p, const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv,
-                   const FwdInt4Args& a, dim3 grid, cudaStream_t cs) {
-  constexpr int smem = SmemInt4<D>::TOTAL;
-  if (p.p_mode == ROTATTN_P_ASYM15) {
-    ROTATTN_CUDA_TRY(cudaFuncSetAttribute(fwd_int4_kernel<D, ROTATTN_P_ASYM15, DEBUG>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    fwd_int4_kernel<D, ROTATTN_P_ASYM15, DEBUG><<<grid, kFwdThreads, smem, cs>>>(tq, tk, tv, a);
-  } else {
-    ROTATTN_CUDA_TRY(cudaFuncSetAttribute(fwd_int4_kernel<D, ROTATTN_P_SYM7, DEBUG>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    fwd_int4_kernel<D, ROTATTN_P_SYM7, DEBUG><<<grid, kFwdThreads, smem, cs>>>(tq, tk, tv, a);
-  }
-  ROTATTN_CUDA_TRY(cudaGetLastError());
-  return ROTATTN_OK;
-}
 
 int fwd_int4_common(const rotattn_params* p, const uint8_t* Q4, const float* Qs, const uint8_t* K4, const float* Ks,
                     const uint8_t* V4, const float* Vs, void* O, const int32_t* head_sel, int32_t n_sel,
                     void* workspace, size_t ws_bytes, int32_t ws_state, void* stream,
-                    bool debug, int32_t bh, int32_t q_tile, int32_t* S_dump, uint8_t* P_dump) {
+                    bool debug, int32_t bh, int32_t q_tile, int32_t* S_dump, uint8_t* P_dump, int32_t* PV_dump) {
   int st = rotattn_validate(p);
   if (st != ROTATTN_OK) return st;
   if (!Q4 || !Qs || !K4 || !Ks || !V4 || !Vs || !O || !workspace) return ROTATTN_ERR_INVALID_ARG;
+  if (((uintptr_t)Vs & 15) || ((uintptr_t)O & 15)) return ROTATTN_ERR_INVALID_ARG;      // bulk copies / 16-byte stores
   const int BH = p->B * p->H;
   const int nblk = ceil_div(p->N, kTile);
   if (head_sel && (n_sel < 1 || n_sel > BH)) return ROTATTN_ERR_INVALID_ARG;
   if (debug && (bh < 0 || bh >= BH || q_tile < 0 || q_tile >= nblk || !S_dump || !P_dump)) return ROTATTN_ERR_INVALID_ARG;
+  if (p->smooth && (ws_state & (ROTATTN_WS_HAS_QK | ROTATTN_WS_HAS_V)) != (ROTATTN_WS_HAS_QK | ROTATTN_WS_HAS_V))
+    return ROTATTN_ERR_INVALID_ARG;     // the smoothing state (means, per-key correction) exists only in the prologue's workspace
   WsInt4 ws(*p);
   if (ws_bytes < ws.total) return ROTATTN_ERR_WORKSPACE_TOO_SMALL;
   if ((st = check_device_sm100()) != ROTATTN_OK) return st;
@@ -501,9 +30,11 @@ int fwd_int4_common(const rotattn_params* p, const uint8_t* Q4, const float* Qs,
   int8_t* q8 = (int8_t*)workspace + ws.q8;
   int8_t* k8 = (int8_t*)workspace + ws.k8;
   int8_t* v8t = (int8_t*)workspace + ws.v8t;
+  float* ksp = (float*)((uint8_t*)workspace + ws.ksp);
   if (!(ws_state & ROTATTN_WS_HAS_QK)) {
     if ((st = launch_unpack_qk(*p, Q4, q8, cs)) != ROTATTN_OK) return st;
     if ((st = launch_unpack_qk(*p, K4, k8, cs)) != ROTATTN_OK) return st;
+    if (p->qk_group == 1 && (st = launch_pad_ks(*p, Ks, ksp, ws.npad, cs)) != ROTATTN_OK) return st;
   }
   if (!(ws_state & ROTATTN_WS_HAS_V)) {
     if ((st = launch_unpack_vt(*p, V4, v8t, ws.npad, cs)) != ROTATTN_OK) return st;
@@ -514,17 +45,16 @@ int fwd_int4_common(const rotattn_params* p, const uint8_t* Q4, const float* Qs,
   if ((st = make_tmap_3d(&tk, k8, 1, kQKRowBytes, N, BH, kQKRowBytes, N * kQKRowBytes, 128, 128)) != ROTATTN_OK) return st;
   if ((st = make_tmap_3d(&tv, v8t, 1, ws.npad, D, BH, ws.npad, D * ws.npad, 128, (uint32_t)D)) != ROTATTN_OK) return st;
   FwdInt4Args a{};
-  a.Qs = Qs; a.Ks = Ks; a.Vs = Vs; a.O = (__half*)O; a.head_sel = head_sel;
-  a.S_dump = S_dump; a.P_dump = P_dump;
+  a.Qs = Qs; a.Ks = Ks; a.KsP = ksp; a.Vs = Vs; a.O = (__half*)O; a.head_sel = head_sel;
+  a.KcP = (const float*)((uint8_t*)workspace + ws.kcp);
+  a.means = (const float*)((uint8_t*)workspace + ws.means);
+  a.S_dump = S_dump; a.P_dump = P_dump; a.PV_dump = PV_dump;
   a.N = p->N; a.nblk = nblk; a.npad = ws.npad; a.dbg_bh = bh; a.dbg_qtile = q_tile;
   a.scale_log2 = (float)(1.4426950408889634 / std::sqrt((double)p->D) * (double)kAccScale);   // S arrives as acc * 2^-18
-#ifdef ROTATTN_TRACE
-  a.trace = g_rotattn_trace;
-#endif
   dim3 grid(debug ? 1 : nblk, debug ? 1 : (head_sel ? n_sel : BH));
   if (p->p_norm == ROTATTN_NORM_RUNNING) return launch_fwd_int4_sync(*p, tq, tk, tv, a, grid, debug, cs);
-  if (p->D == 128) return debug ? launch_variant<128, true>(*p, tq, tk, tv, a, grid, cs) : launch_variant<128, false>(*p, tq, tk, tv, a, grid, cs);
-  return debug ? launch_variant<64, true>(*p, tq, tk, tv, a, grid, cs) : launch_variant<64, false>(*p, tq, tk, tv, a, grid, cs);
+  if (debug) return launch_fwd_int4_debug(*p, tq, tk, tv, a, grid, cs);
+  return p->D == 128 ? launch_fwd_int4_d128(*p, tq, tk, tv, a, grid, cs) : launch_fwd_int4_d64(*p, tq, tk, tv, a, grid, cs);
 }
 
 }  // namespace
@@ -533,13 +63,13 @@ extern "C" int rotattn_fwd_int4(const rotattn_params* p, const uint8_t* Q4, cons
                                 const float* Ks, const uint8_t* V4, const float* Vs, void* O, const int32_t* head_sel,
                                 int32_t n_sel, void* workspace, size_t ws_bytes, int32_t ws_state, void* stream) {
   return fwd_int4_common(p, Q4, Qs, K4, Ks, V4, Vs, O, head_sel, n_sel, workspace, ws_bytes, ws_state, stream,
-                         false, 0, 0, nullptr, nullptr);
+                         false, 0, 0, nullptr, nullptr, nullptr);
 }
 
 extern "C" int rotattn_fwd_int4_debug(const rotattn_params* p, const uint8_t* Q4, const float* Qs, const uint8_t* K4,
                                       const float* Ks, const uint8_t* V4, const float* Vs, int32_t bh, int32_t q_tile,
-                                      int32_t* S_dump, uint8_t* P_dump, void* O_tile, void* workspace, size_t ws_bytes,
-                                      int32_t ws_state, void* stream) {
+                                      int32_t* S_dump, uint8_t* P_dump, int32_t* PV_dump, void* O_tile, void* workspace,
+                                      size_t ws_bytes, int32_t ws_state, void* stream) {
   return fwd_int4_common(p, Q4, Qs, K4, Ks, V4, Vs, O_tile, nullptr, 0, workspace, ws_bytes, ws_state, stream,
-                         true, bh, q_tile, S_dump, P_dump);
+                         true, bh, q_tile, S_dump, P_dump, PV_dump);
 }

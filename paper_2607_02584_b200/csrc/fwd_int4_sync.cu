@@ -1,7 +1,7 @@
 // fwd_int4_sync: INT4 FlashAttention forward with the softmax serialised over KV blocks (2 threads per query row,
 // running max kept by the softmax threads).  Used for p_norm = RUNNING (codes relative to the running max,
 // SURVEY 8c reading 13 alternative), where block j cannot be normalised before block j-1 is known.
-// Same tcgen05 kind::i8 / TMA / TMEM structure as fwd_int4.cu.
+// Same operand path as fwd_int4_kernel.cuh: tcgen05 kind::f8f6f4 on integer-exact E4M3 code bytes, TMA, TMEM.
 #include <cmath>
 #include <cstdio>
 #include "fwd_int4.cuh"

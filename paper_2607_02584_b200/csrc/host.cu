@@ -40,11 +40,16 @@ int rotattn_validate(const rotattn_params* p) {
   if (p->D != 64 && p->D != 128) return ROTATTN_ERR_UNSUPPORTED;
   if (p->pairs_t + p->pairs_h + p->pairs_w != p->D / 2) return ROTATTN_ERR_INVALID_ARG;
   if (!(p->rope_base > 1.0f)) return ROTATTN_ERR_INVALID_ARG;
-  if (p->rot_mode < 0 || p->rot_mode > 2) return ROTATTN_ERR_INVALID_ARG;
+  if (p->rot_mode < 0 || p->rot_mode > 3) return ROTATTN_ERR_INVALID_ARG;
   if (p->p_mode < 0 || p->p_mode > 1) return ROTATTN_ERR_INVALID_ARG;
   if (p->p_norm < 0 || p->p_norm > 1) return ROTATTN_ERR_INVALID_ARG;
-  if (p->qk_group != 1) return ROTATTN_ERR_UNSUPPORTED;
+  if (p->v_scale < 0 || p->v_scale > 1 || p->smooth < 0 || p->smooth > 1 || p->qk_group < 1) return ROTATTN_ERR_INVALID_ARG;
+  if (p->qk_group != 1 && p->qk_group != kTile) return ROTATTN_ERR_UNSUPPORTED;
   if (p->v_group != kTile || p->kv_block != kTile) return ROTATTN_ERR_UNSUPPORTED;
+  // the RUNNING normaliser and smoothing are built for the paper's granularity only (per-token Q/K, per-channel V scales)
+  const bool f1 = p->qk_group != 1 || p->v_scale != ROTATTN_VSCALE_CHANNEL;
+  if (f1 && (p->p_norm == ROTATTN_NORM_RUNNING || p->smooth)) return ROTATTN_ERR_UNSUPPORTED;
+  if (p->smooth && p->p_norm == ROTATTN_NORM_RUNNING) return ROTATTN_ERR_UNSUPPORTED;
   return ROTATTN_OK;
 }
 
@@ -109,8 +114,8 @@ int rotattn_build_tables(const rotattn_params* p, const float* rot_host, float* 
 
 size_t rotattn_workspace_bytes(const rotattn_params* p, int which) {
   if (rotattn_validate(p) != ROTATTN_OK) return 0;
-  if (which == 0) return WsInt4(*p).total;
-  if (which == 1) return WsFp16(*p).total;
+  if (which == 0 || which == 1) return WsInt4(*p).total;      // prepare_qk / quant_v and fwd_int4 share one workspace
+  if (which == 2) return WsFp16(*p).total;
   return 0;
 }
 
@@ -120,13 +125,17 @@ int rotattn_policy_select(const rotattn_policy* pol, int32_t step, int32_t block
   if (pol->first_steps < 0 || pol->last_steps < 0 || pol->first_blocks < 0 || pol->last_blocks < 0) return ROTATTN_ERR_INVALID_ARG;
   if (step < pol->first_steps || step >= pol->n_steps - pol->last_steps) return 1;
   if (block < pol->first_blocks || block >= pol->n_blocks - pol->last_blocks) return 1;
-  if (pol->fp16_head_mask && pol->fp16_head_mask[head]) return 1;
+  if (pol->fp16_head_mask) {
+    if (head >= pol->n_heads) return ROTATTN_ERR_INVALID_ARG;      // the mask holds n_heads entries
+    if (pol->fp16_head_mask[head]) return 1;
+  }
   return 0;
 }
 
 int rotattn_policy_split_heads(const rotattn_policy* pol, int32_t step, int32_t block, int32_t B, int32_t H,
                                int32_t* sel_int4, int32_t* n_int4, int32_t* sel_fp16, int32_t* n_fp16) {
-  if (!sel_int4 || !n_int4 || !sel_fp16 || !n_fp16 || B < 1 || H < 1) return ROTATTN_ERR_INVALID_ARG;
+  if (!pol || !sel_int4 || !n_int4 || !sel_fp16 || !n_fp16 || B < 1 || H < 1) return ROTATTN_ERR_INVALID_ARG;
+  if (pol->fp16_head_mask && H > pol->n_heads) return ROTATTN_ERR_INVALID_ARG;
   int a = 0, b = 0;
   for (int bi = 0; bi < B; ++bi)
     for (int h = 0; h < H; ++h) {

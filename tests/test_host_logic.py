@@ -18,7 +18,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def test_header_symbols_exported():
-    hdr = open(os.path.join(ROOT, 'include', 'rotattn.h')).read()
+    hdr = open(os.path.join(ROOT, 'include', 'rotattn.h')).read() + open(os.path.join(ROOT, 'include', 'rotattn_debug.h')).read()
     names = set(re.findall(r'\b(rotattn_[a-z0-9_]+)\s*\(', hdr))
     assert names == set(b.EXPORTS), names ^ set(b.EXPORTS)
     for n in names:
@@ -40,7 +40,12 @@ def test_validate_codes():
     bad = _p(w); bad.D = 96; bad.pairs_t = 28
     assert b.lib.rotattn_validate(C.byref(bad)) == -2
     assert b.lib.rotattn_validate(C.byref(_p(w, kv_block=64))) == -2
-    assert b.lib.rotattn_validate(C.byref(_p(w, qk_group=128))) == -2
+    assert b.lib.rotattn_validate(C.byref(_p(w, qk_group=128))) == 0          # f1: one scale per 128-token block
+    assert b.lib.rotattn_validate(C.byref(_p(w, qk_group=64))) == -2
+    assert b.lib.rotattn_validate(C.byref(_p(w, qk_group=128, p_norm=b.NORM_RUNNING))) == -2
+    assert b.lib.rotattn_validate(C.byref(_p(w, v_scale=b.VSCALE_GROUP, smooth=1))) == -2
+    assert b.lib.rotattn_validate(C.byref(_p(w, v_scale=2))) == -1
+    assert b.lib.rotattn_validate(C.byref(_p(w, rot_mode=b.ROT_FULL, smooth=1))) == 0
     assert b.lib.rotattn_strerror(-3).decode().startswith('rotation')
 
 
@@ -81,13 +86,14 @@ def test_workspace_sizes():
     npad = -(-w.N // 128) * 128
     ws0 = b.lib.rotattn_workspace_bytes(C.byref(p), 0)
     assert ws0 >= 2 * w.H * w.N * 128 + w.H * w.D * npad
-    assert b.lib.rotattn_workspace_bytes(C.byref(p), 1) >= w.H * w.D * npad * 2
+    assert b.lib.rotattn_workspace_bytes(C.byref(p), 1) == ws0        # prepare_qk / quant_v and fwd_int4 share one workspace
+    assert b.lib.rotattn_workspace_bytes(C.byref(p), 2) >= w.H * w.D * npad * 2
     assert b.lib.rotattn_workspace_bytes(C.byref(p), 7) == 0
 
 
 def test_policy_matches_oracle_and_paper_fractions():
     for ns, nb, fs, ls, fb, lb in [(40, 40, 6, 4, 2, 2), (40, 40, 2, 2, 2, 2), (50, 60, 4, 2, 2, 2)]:
-        pol = b.RotattnPolicy(ns, nb, fs, ls, fb, lb, None)
+        pol = b.RotattnPolicy(ns, nb, fs, ls, fb, lb, 0, None)
         o = orc.Policy(ns, nb, fs, ls, fb, lb)
         n = 0
         for s in range(ns):
@@ -96,12 +102,14 @@ def test_policy_matches_oracle_and_paper_fractions():
                 assert r == o.select(s, k)
                 n += 1 - r
         assert n / (ns * nb) == o.int4_fraction()
-    assert b.lib.rotattn_policy_select(C.byref(b.RotattnPolicy(40, 40, 2, 2, 2, 2, None)), 40, 0, 0) == -1
+    assert b.lib.rotattn_policy_select(C.byref(b.RotattnPolicy(40, 40, 2, 2, 2, 2, 0, None)), 40, 0, 0) == -1
 
 
 def test_policy_split_heads():
     mask = (C.c_uint8 * 6)(0, 1, 0, 0, 1, 0)
-    pol = b.RotattnPolicy(50, 4, 5, 0, 0, 0, mask)
+    pol = b.RotattnPolicy(50, 4, 5, 0, 0, 0, 6, mask)
+    assert b.lib.rotattn_policy_select(C.byref(pol), 7, 0, 5) == 0
+    assert b.lib.rotattn_policy_select(C.byref(pol), 7, 0, 6) == -1          # head beyond the mask: error, not a stray read
     a = np.zeros(12, dtype=np.int32); bb = np.zeros(12, dtype=np.int32)
     na, nb = C.c_int32(), C.c_int32()
     args = (a.ctypes.data_as(C.c_void_p), C.cast(C.byref(na), C.c_void_p), bb.ctypes.data_as(C.c_void_p), C.cast(C.byref(nb), C.c_void_p))
@@ -109,6 +117,7 @@ def test_policy_split_heads():
     assert na.value == 0 and nb.value == 12
     assert b.lib.rotattn_policy_split_heads(C.byref(pol), 7, 1, 2, 6, *args) == 0
     assert list(a[:na.value]) == [0, 2, 3, 5, 6, 8, 9, 11] and list(bb[:nb.value]) == [1, 4, 7, 10]
+    assert b.lib.rotattn_policy_split_heads(C.byref(pol), 7, 1, 2, 7, *args) == -1      # H larger than the mask
 
 
 def test_compute_entry_points_fail_loudly_without_gpu():
