@@ -24,8 +24,9 @@ reproducible bit for bit.  Softmax arithmetic is fp64.
 
 Pins: tests/test_oracle_pins.py (-m "not gpu").  Parity status per function:
   hadamard, h2, token_positions (golden triples on an asymmetric grid), rope, coef_table,
-  apply_rope_rot, quantisers, pack/unpack, integer products, P codes, online softmax,
-  policy : pinned (see that file).
+  apply_rope_rot (incl. the FULL butterfly), quantisers (per-token / per-block / per-group),
+  pack/unpack, integer products, P codes, online softmax, smoothing (column_mean_fixed,
+  exactness of the K / Q / V shifts), policy : pinned (see that file).
   INT4-vs-exact *quality numbers* : parity unpinned (paper gives only video-level
   metrics on real weights, Table 1); reported, never asserted.
 """
@@ -36,9 +37,10 @@ from dataclasses import dataclass, field
 
 import numpy as np
 
-ROT_NONE, ROT_INTERLEAVED, ROT_HALF = 0, 1, 2
+ROT_NONE, ROT_INTERLEAVED, ROT_HALF, ROT_FULL = 0, 1, 2, 3
 P_ASYM15, P_SYM7 = 0, 1
 NORM_ROWBLOCK, NORM_RUNNING = 0, 1
+VSCALE_CHANNEL, VSCALE_GROUP = 0, 1
 
 F32 = np.float32
 F64 = np.float64
@@ -60,6 +62,8 @@ class Params:
     qk_group: int = 1      # tokens per Q/K scale; 1 = per-token (L190)
     v_group: int = 128     # tokens per V scale group (L190 "per-group"; reading 11)
     kv_block: int = 128    # FlashAttention KV block (L157; reading 18)
+    v_scale: int = VSCALE_CHANNEL   # one V scale per (group, channel) (reading 11) | one per group
+    smooth: int = 0        # subtract the token mean of Q, K, V before quantisation (L90, L40, L52)
 
     @property
     def n_rope(self):
@@ -203,7 +207,27 @@ def apply_rope_rot(p: Params, x16, coef, rot=None):
             y[:, o + P:o + 2 * P] = (u * rr[:, 1]).astype(F32) + (v * rr[:, 3]).astype(F32)
             o += 2 * P
             g += P
+    if p.rot_mode == ROT_FULL:
+        y = fwht_fp32(y)
     return y
+
+
+def fwht_fp32(y):
+    """The paper's "Full" rotation baseline (L208: a dense D x D Hadamard applied online after RoPE): y <- y H_D / sqrt(D),
+    evaluated as the Sylvester butterfly of Eq.13 (H_{2^n} = H_2 (x) H_{2^{n-1}}) in fp32, one rounding per operation:
+    strides 1, 2, ..., D/2 in this order, (a, b) -> (a + b, a - b) with a the lower channel, then one multiplication by
+    fl32(1/sqrt(D)).  Pinned against the dense product with hadamard(D) in tests/test_oracle_pins.py."""
+    y = np.array(y, dtype=F32, copy=True)
+    N, D = y.shape
+    s = 1
+    while s < D:
+        v = y.reshape(N, D // (2 * s), 2, s)
+        a, b = v[:, :, 0, :].copy(), v[:, :, 1, :].copy()
+        v[:, :, 0, :] = (a + b).astype(F32)
+        v[:, :, 1, :] = (a - b).astype(F32)
+        y = v.reshape(N, D)
+        s *= 2
+    return (y * F32(1.0 / math.sqrt(D))).astype(F32)
 
 
 def rope_fp64(p: Params, x, rot_mode=ROT_NONE, rot=None):
@@ -249,6 +273,8 @@ def dense_rotation(p: Params, rot_mode, rot=None):
                 R[b, a], R[b, b] = blk[1, 0], blk[1, 1]
             o += 2 * P
             g += P
+    elif rot_mode == ROT_FULL:
+        R = hadamard(D)
     else:
         R = np.eye(D)
     return R
@@ -289,22 +315,56 @@ def quant_qk(y, qk_group=1):
     return codes, scales
 
 
-def quant_v(v16, v_group=128):
+def quant_v(v16, v_group=128, v_scale=VSCALE_CHANNEL, mean=None):
     """Per-group INT4 of Hadamard-domain V (L190 "per-group quantization for V"): one scale per
     (group of v_group consecutive tokens, channel); ragged last group uses the tokens that exist.
-    v16 fp16 [N,D] -> codes int8 [N,D], scales fp32 [ceil(N/v_group), D]."""
+    v_scale = VSCALE_GROUP: one scale per group (amax over the group's tokens AND channels).
+    mean (smoothing, fp32 [D]): v - mean is quantised (one fp32 subtraction per element).
+    v16 fp16 [N,D] -> codes int8 [N,D], scales fp32 [ceil(N/v_group), D]  (VSCALE_GROUP: [ceil(N/v_group)])."""
     N, D = v16.shape
     v = v16.astype(F32)
+    if mean is not None:
+        v = (v - np.asarray(mean, dtype=F32)[None, :]).astype(F32)
     ng = -(-N // v_group)
     codes = np.empty((N, D), dtype=np.int8)
-    scales = np.empty((ng, D), dtype=F32)
+    scales = np.empty((ng, D) if v_scale == VSCALE_CHANNEL else (ng,), dtype=F32)
     for g in range(ng):
         sl = slice(g * v_group, min(N, (g + 1) * v_group))
-        amax = np.abs(v[sl]).max(axis=0)
-        c, s = _quant_sym7(v[sl], amax[None, :])
+        if v_scale == VSCALE_CHANNEL:
+            amax = np.abs(v[sl]).max(axis=0)
+            c, s = _quant_sym7(v[sl], amax[None, :])
+            scales[g] = s[0]
+        else:
+            amax = np.abs(v[sl]).max()
+            c, s = _quant_sym7(v[sl], np.full((1, 1), amax, dtype=F32))
+            scales[g] = s[0, 0]
         codes[sl] = c
-        scales[g] = s[0]
     return codes, scales
+
+
+# ----------------------------------------------------------------------------------
+# Smoothing (L90 "we first perform smoothing on Q, K, V"; L40 Q - E[Q]; L52): SURVEY 8f row f2
+# ----------------------------------------------------------------------------------
+FIX_QK = 2.0 ** 20      # fixed-point unit of the column sums of y_Q, y_K
+FIX_V = 2.0 ** 24       # fp16 V is a multiple of 2^-24, so its fixed-point sum is exact
+
+
+def column_mean_fixed(x32, unit):
+    """Token mean of every channel, defined through a fixed-point sum so that it does not depend on the order of
+    summation (the GPU adds in parallel):  mean = fl32( fp64(sum_n rne(x_n * unit)) / (N * unit) ).
+    x32 fp32 [N,D] -> fp32 [D]."""
+    x32 = np.asarray(x32, dtype=F32)
+    fx = np.rint((x32 * F32(unit)).astype(F32).astype(F64)).astype(np.int64)
+    tot = fx.sum(axis=0)                                   # exact integer sums
+    return (tot.astype(F64) / (F64(x32.shape[0]) * F64(unit))).astype(F32)
+
+
+def smooth_means(p: Params, q16, k16, v16, coef, rot=None):
+    """Column means of y_Q, y_K (after RoPE and rotation, the tensors that are quantised) and of V."""
+    yq = apply_rope_rot(p, q16, coef, rot)
+    yk = apply_rope_rot(p, k16, coef, rot)
+    return (column_mean_fixed(yq, FIX_QK), column_mean_fixed(yk, FIX_QK),
+            column_mean_fixed(v16.astype(F32), FIX_V))
 
 
 def pack_nibbles(codes):
@@ -330,18 +390,24 @@ def unpack_nibbles(packed):
 # ----------------------------------------------------------------------------------
 # Prologue = steps a1-a3 for one head
 # ----------------------------------------------------------------------------------
-def prepare_qk_head(p: Params, q16, k16, coef, rot=None):
+def prepare_qk_head(p: Params, q16, k16, coef, rot=None, means=None):
     """One head: RoPE o R in fp32 then per-token INT4.  Returns dict with y (fp32), fp16 copy,
-    codes, packed codes, scales for Q and K."""
+    codes, packed codes, scales for Q and K.
+    means = (mean_q, mean_k) (smoothing): y - mean is quantised (one fp32 subtraction per element); k_corr[j] =
+    mean_q . (y_K[j] - mean_k) is the rank-1 term that fwd adds back to S (exact: (Q' + 1 mean_q^T) K'^T)."""
     out = {}
     for name, x in (('q', q16), ('k', k16)):
         y = apply_rope_rot(p, x, coef, rot)
+        out[name + '_16'] = y.astype(np.float16)            # the FP16 path is never smoothed
+        if means is not None:
+            y = (y - np.asarray(means[0 if name == 'q' else 1], dtype=F32)[None, :]).astype(F32)
         codes, scale = quant_qk(y, p.qk_group)
         out[name + '_y'] = y
-        out[name + '_16'] = y.astype(np.float16)
         out[name + '_codes'] = codes
         out[name + '_packed'] = pack_nibbles(codes)
         out[name + '_scale'] = scale
+    if means is not None:
+        out['k_corr'] = out['k_y'].astype(F64) @ np.asarray(means[0], dtype=F64)
     return out
 
 
@@ -374,7 +440,7 @@ def p_codes_block(s_blk, m_ref, p_mode):
 
 
 def o_quant(p: Params, qc, qs, kc, ks, vc, vs, rows=None, dump=False, quantize=True,
-            p_mode=None, p_norm=None):
+            p_mode=None, p_norm=None, k_corr=None, v_mean=None, dump_pv=False):
     """Steps 7-12 for one head, fp64 softmax arithmetic.
     qc,kc,vc: int8 codes [N,D]; qs,ks: fp32 scales [ceil(N/qk_group)]; vs: fp32 [nG, D].
     rows: query rows to evaluate (default all).  quantize=False switches every quantiser of the
@@ -393,6 +459,9 @@ def o_quant(p: Params, qc, qs, kc, ks, vc, vs, rows=None, dump=False, quantize=T
     # step 7: integer scores; fp64 BLAS on integer-valued codes is exact (|acc| <= 49 D << 2^53)
     acc = q @ kc.astype(F64).T                         # [R, N] integers
     s = acc * qscale[:, None] * kscale[None, :] / math.sqrt(D)
+    if k_corr is not None:      # smoothing: rank-1 correction mean(Q) K'^T added to S in floating point
+        s = s + np.asarray(k_corr, dtype=F64)[None, :] / math.sqrt(D)
+    pv_dump = [] if dump_pv else None
     m = np.full(Rn, -np.inf)
     l = np.zeros(Rn)
     O = np.zeros((Rn, D))
@@ -412,13 +481,15 @@ def o_quant(p: Params, qc, qs, kc, ks, vc, vs, rows=None, dump=False, quantize=T
         alpha = np.exp(m - m_new)                      # exp(-inf) = 0 on the first block
         vblk = vc[j0:j1].astype(F64)
         g = j0 // p.v_group
-        vscale = vs[g].astype(F64)                     # [D]
+        vscale = np.broadcast_to(np.asarray(vs[g], dtype=F64), (vc.shape[1],))      # [D] (one value repeated for VSCALE_GROUP)
         if quantize:
             pv = u @ vblk                              # step 10, unsigned form
             # signed form with zero-point -8 (L166): sum (u-8) v + 8 sum v — must be the same integer
             pv_signed = (u - 8.0) @ vblk + 8.0 * vblk.sum(axis=0)[None, :]
             assert np.array_equal(pv, pv_signed), "zero-point identity violated"
             contrib = pv * (vscale / levels)[None, :]
+            if dump_pv:
+                pv_dump.append(pv.astype(np.int64))
         else:
             contrib = phat @ (vblk * vscale[None, :])
         l = alpha * l + beta * phat.sum(axis=1)        # un-rounded P^ (reading 16)
@@ -427,6 +498,10 @@ def o_quant(p: Params, qc, qs, kc, ks, vc, vs, rows=None, dump=False, quantize=T
         if dump:
             codes_dump[:, j0:j1] = u.astype(np.int16)
     O = O / l[:, None]                                 # step 12
+    if v_mean is not None:      # smoothing: softmax(.)(V - 1 mean^T) + mean^T = softmax(.) V
+        O = O + np.asarray(v_mean, dtype=F64)[None, :]
+    if dump_pv:
+        return O, acc.astype(np.int32), codes_dump, np.stack(pv_dump)
     if dump:
         return O, acc.astype(np.int32), codes_dump
     return O
@@ -484,11 +559,13 @@ class Policy:
 # ----------------------------------------------------------------------------------
 # Full pipeline for one head (used by tests / bench cpu_baseline)
 # ----------------------------------------------------------------------------------
-def int4_attention_head(p: Params, q16, k16, v16, rot=None, rows=None, dump=False):
+def int4_attention_head(p: Params, q16, k16, v16, rot=None, rows=None, dump=False, coef=None):
     """prologue + o_quant for one head from fp16 inputs (V already in the Hadamard domain)."""
-    coef = coef_table(p, rot)
-    pq = prepare_qk_head(p, q16, k16, coef, rot)
-    vc, vs = quant_v(v16, p.v_group)
+    coef = coef_table(p, rot) if coef is None else coef
+    means = smooth_means(p, q16, k16, v16, coef, rot) if p.smooth else None
+    pq = prepare_qk_head(p, q16, k16, coef, rot, means=None if means is None else means[:2])
+    vc, vs = quant_v(v16, p.v_group, p.v_scale, mean=None if means is None else means[2])
     res = o_quant(p, pq['q_codes'], pq['q_scale'], pq['k_codes'], pq['k_scale'], vc, vs,
-                  rows=rows, dump=dump)
+                  rows=rows, dump=dump, k_corr=pq.get('k_corr'), v_mean=None if means is None else means[2])
+    pq['means'] = means
     return res, pq, (vc, vs)

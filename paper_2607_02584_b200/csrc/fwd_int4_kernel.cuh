@@ -57,7 +57,8 @@ struct SmemInt4 {
   static constexpr int P_BYTES = 128 * 128;                           // u8 codes [128 query rows][128 keys], 128-byte swizzle
   static constexpr int OFF_P = OFF_V + V_STAGES * V_BYTES;
   static constexpr int OFF_KS = OFF_P + P_SLOTS * P_BYTES;            // float [KS_RING][128]
-  static constexpr int OFF_VS = OFF_KS + KS_RING * 128 * 4;           // float [VS_RING][D]
+  static constexpr int OFF_KC = OFF_KS + KS_RING * 128 * 4;           // float [KS_RING][128]  smoothing: per-key correction
+  static constexpr int OFF_VS = OFF_KC + KS_RING * 128 * 4;           // float [VS_RING][D]
   static constexpr int OFF_AB = OFF_VS + VS_RING * D * 4;             // float [AB_RING][3][128]: block max, half-row sums of the two key halves
   static constexpr int OFF_MX = OFF_AB + AB_RING * 3 * 128 * 4;       // float [2 groups][2 parities][2 halves][128]
   static constexpr int OFF_BAR = OFF_MX + 2 * 2 * 2 * 128 * 4;        // mbarriers
@@ -70,13 +71,15 @@ struct SmemInt4 {
 // Pass 1.  SCALE (per-token Q/K scales): t = S * (Ks_j * 2^18 log2e/sqrt(D)) (the query scale Qs_i > 0 is applied after
 // the max), returned for the write-back over S so that pass 2 needs neither the key scales nor the mask.
 // !SCALE (one K scale per block): bare max over the raw accumulators.  Keys >= N are masked to -inf.
-template <bool SCALE, bool MASK>
-__device__ __forceinline__ void chunk_scale_max(const uint32_t (&v)[16], const float2* ks2, int nvalid_rel, uint32_t (&t)[16],
-                                                float& mx0, float& mx1) {
+// BIAS (smoothing): t = S * Ks_j * Qs_i + kc_j, the per-key rank-1 correction mean(Q) . K'_j in the log2 domain.
+template <bool SCALE, bool BIAS, bool MASK>
+__device__ __forceinline__ void chunk_scale_max(const uint32_t (&v)[16], const float2* ks2, const float2* kc2, float2 qs2,
+                                                int nvalid_rel, uint32_t (&t)[16], float& mx0, float& mx1) {
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
     float2 t2 = make_float2(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1]));
     if (SCALE) t2 = fmul2(t2, ks2[i]);
+    if (BIAS) t2 = ffma2(t2, qs2, kc2[i]);
     if (MASK) {
       if (2 * i >= nvalid_rel) t2.x = -INFINITY;
       if (2 * i + 1 >= nvalid_rel) t2.y = -INFINITY;
@@ -117,7 +120,7 @@ __device__ __forceinline__ void chunk_exp(const uint32_t (&t)[16], float2 qs2, f
   }
 }
 
-template <int D, int P_MODE, int QKG, int VSC, bool DEBUG>
+template <int D, int P_MODE, int QKG, int VSC, int SM, bool DEBUG>
 __global__ void __launch_bounds__(kFwdThreads, 1)
 fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                 const __grid_constant__ CUtensorMap tmV, const FwdInt4Args a) {
@@ -128,6 +131,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   uint8_t* sV = smem + L::OFF_V;
   uint8_t* sP = smem + L::OFF_P;
   float* sKs = (float*)(smem + L::OFF_KS);
+  float* sKc = (float*)(smem + L::OFF_KC);
   float* sVs = (float*)(smem + L::OFF_VS);
   float* sAB = (float*)(smem + L::OFF_AB);
   float* sMx = (float*)(smem + L::OFF_MX);
@@ -262,12 +266,13 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       if (QKG == 1 || VSC == 0) {
         for (int j = 0; j < nblk; ++j) {
           const int s = j % KS_RING;
-          float kv[4], vv[D / 32];
+          float kv[4], kc[4], vv[D / 32];
           if (QKG == 1) {
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
               const int kj = j * kTile + i * 32 + lane;
               kv[i] = (kj < a.N) ? ksrc[kj] * a.scale_log2 : 0.f;
+              if (SM) kc[i] = (kj < a.N) ? a.KcP[(size_t)bh * a.npad + kj] : 0.f;
             }
           }
           if (VSC == 0) {
@@ -277,7 +282,10 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           if (QKG == 1) {
             mbar_wait(&ks_empty[s], ((j / KS_RING) & 1) ^ 1);
 #pragma unroll
-            for (int i = 0; i < 4; ++i) sKs[s * 128 + i * 32 + lane] = kv[i];
+            for (int i = 0; i < 4; ++i) {
+              sKs[s * 128 + i * 32 + lane] = kv[i];
+              if (SM) sKc[s * 128 + i * 32 + lane] = kc[i];
+            }
             mbar_arrive(&ks_full[s]);
           }
           if (VSC == 0) {
@@ -310,6 +318,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       const int n = j >> 1;
       const int ring = j % KS_RING, slot = j % P_SLOTS, abslot = j % AB_RING;
       const float2* ks2 = reinterpret_cast<const float2*>(sKs + ring * 128 + cb);
+      const float2* kc2 = reinterpret_cast<const float2*>(sKc + ring * 128 + cb);
       const int nvalid = min(kTile, a.N - j * kTile) - cb;   // valid keys of this half; < 64 only on the ragged last block
       const bool ragged = nvalid < 64;
       float qs = fq;
@@ -335,7 +344,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             for (int i = 0; i < 16; ++i)
               a.S_dump[(size_t)r * a.npad + j * kTile + cb + c * 16 + i] = (int32_t)(__uint_as_float(cur[i]) * kAccScale);
           }
-          chunk_scale_max<QKG == 1, decltype(masked)::value>(cur, ks2 + c * 8, nvalid - c * 16, tt, mx0, mx1);
+          chunk_scale_max<QKG == 1, SM != 0, decltype(masked)::value>(cur, ks2 + c * 8, kc2 + c * 8, qs2, nvalid - c * 16, tt, mx0, mx1);
           if (QKG == 1) tmem_st16(s_addr + c * 16, tt);
         }
       };
@@ -350,7 +359,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       }
       bar_sync(pair_bar, 64);
       tmax = fmaxf(tmax, mxbuf[(h ^ 1) * 128 + r]);
-      const float mt = qs * tmax;                        // block row max of s * log2e
+      const float mt = SM ? tmax : qs * tmax;            // block row max of s * log2e (smoothing: Qs_i is already in t)
       const float nref = LOG2_LEVELS - mt;
       const float2 nref2 = make_float2(nref, nref);
       mbar_wait(&pv_done[slot], ((j / P_SLOTS) & 1) ^ 1);            // P~V(j-4) has consumed this P slot
@@ -366,7 +375,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           if (c < 3) tmem_ld16(s_addr + (c + 1) * 16, nxt);
           else { tc_fence_before(); mbar_arrive(&s_empty[g]); }          // this thread is done with the S buffer
           uint32_t pw[4];
-          chunk_exp<decltype(masked)::value>(cur, qs2, nref2, nvalid - c * 16, ls0, ls1, pw);
+          chunk_exp<decltype(masked)::value>(cur, SM ? make_float2(1.f, 1.f) : qs2, nref2, nvalid - c * 16, ls0, ls1, pw);
           if (DEBUG) {
 #pragma unroll
             for (int q = 0; q < 4; ++q) *reinterpret_cast<uint32_t*>(a.P_dump + (size_t)r * a.npad + j * kTile + cb + c * 16 + q * 4) = pw[q];
@@ -451,11 +460,16 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     const float inv_l = 1.f / l_run;
     if (row < a.N) {
       __half* dst = (DEBUG ? a.O + (size_t)r * D : a.O + ((size_t)bh * a.N + row) * D) + h * DH;
+      const float2* mv2 = reinterpret_cast<const float2*>(a.means + ((size_t)bh * 3 + 2) * D + h * DH);   // smoothing: mean of V
 #pragma unroll
       for (int d = 0; d < DH; d += 8) {
         __half2 hh[4];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) hh[i] = __floats2half2_rn(o2[d / 2 + i].x * inv_l, o2[d / 2 + i].y * inv_l);
+        for (int i = 0; i < 4; ++i) {
+          float2 o = make_float2(o2[d / 2 + i].x * inv_l, o2[d / 2 + i].y * inv_l);
+          if (SM) { const float2 m = mv2[d / 2 + i]; o.x += m.x; o.y += m.y; }       // softmax(.)(V - mean) + mean
+          hh[i] = __floats2half2_rn(o.x, o.y);
+        }
         *reinterpret_cast<uint4*>(dst + d) = *reinterpret_cast<uint4*>(hh);
       }
     }
@@ -467,11 +481,11 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 
 
 // ---- host side: variant dispatch for one (D, DEBUG) flavour -------------------------------------------------------
-template <int D, int P_MODE, int QKG, int VSC, bool DEBUG>
+template <int D, int P_MODE, int QKG, int VSC, int SM, bool DEBUG>
 int launch_one(const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv, const FwdInt4Args& a, dim3 grid,
                cudaStream_t cs) {
   constexpr int smem = SmemInt4<D>::TOTAL;
-  auto kern = fwd_int4_kernel<D, P_MODE, QKG, VSC, DEBUG>;
+  auto kern = fwd_int4_kernel<D, P_MODE, QKG, VSC, SM, DEBUG>;
   static int checked = 0;       // once per variant: ptxas must have allocated exactly the register pool setmaxnreg assumes
   if (!checked) {
     cudaFuncAttributes fa;
@@ -492,15 +506,18 @@ template <int D, bool DEBUG>
 int launch_variants(const rotattn_params& p, const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv,
                     const FwdInt4Args& a, dim3 grid, cudaStream_t cs) {
   const int sel = (p.p_mode == ROTATTN_P_SYM7 ? 4 : 0) | (p.qk_group == 128 ? 2 : 0) | (p.v_scale == ROTATTN_VSCALE_GROUP ? 1 : 0);
+  if (p.smooth)        // validated: smoothing comes with the paper's granularity only
+    return sel & 4 ? launch_one<D, ROTATTN_P_SYM7, 1, 0, 1, DEBUG>(tq, tk, tv, a, grid, cs)
+                   : launch_one<D, ROTATTN_P_ASYM15, 1, 0, 1, DEBUG>(tq, tk, tv, a, grid, cs);
   switch (sel) {
-    case 0: return launch_one<D, ROTATTN_P_ASYM15, 1, 0, DEBUG>(tq, tk, tv, a, grid, cs);
-    case 1: return launch_one<D, ROTATTN_P_ASYM15, 1, 1, DEBUG>(tq, tk, tv, a, grid, cs);
-    case 2: return launch_one<D, ROTATTN_P_ASYM15, 128, 0, DEBUG>(tq, tk, tv, a, grid, cs);
-    case 3: return launch_one<D, ROTATTN_P_ASYM15, 128, 1, DEBUG>(tq, tk, tv, a, grid, cs);
-    case 4: return launch_one<D, ROTATTN_P_SYM7, 1, 0, DEBUG>(tq, tk, tv, a, grid, cs);
-    case 5: return launch_one<D, ROTATTN_P_SYM7, 1, 1, DEBUG>(tq, tk, tv, a, grid, cs);
-    case 6: return launch_one<D, ROTATTN_P_SYM7, 128, 0, DEBUG>(tq, tk, tv, a, grid, cs);
-    default: return launch_one<D, ROTATTN_P_SYM7, 128, 1, DEBUG>(tq, tk, tv, a, grid, cs);
+    case 0: return launch_one<D, ROTATTN_P_ASYM15, 1, 0, 0, DEBUG>(tq, tk, tv, a, grid, cs);
+    case 1: return launch_one<D, ROTATTN_P_ASYM15, 1, 1, 0, DEBUG>(tq, tk, tv, a, grid, cs);
+    case 2: return launch_one<D, ROTATTN_P_ASYM15, 128, 0, 0, DEBUG>(tq, tk, tv, a, grid, cs);
+    case 3: return launch_one<D, ROTATTN_P_ASYM15, 128, 1, 0, DEBUG>(tq, tk, tv, a, grid, cs);
+    case 4: return launch_one<D, ROTATTN_P_SYM7, 1, 0, 0, DEBUG>(tq, tk, tv, a, grid, cs);
+    case 5: return launch_one<D, ROTATTN_P_SYM7, 1, 1, 0, DEBUG>(tq, tk, tv, a, grid, cs);
+    case 6: return launch_one<D, ROTATTN_P_SYM7, 128, 0, 0, DEBUG>(tq, tk, tv, a, grid, cs);
+    default: return launch_one<D, ROTATTN_P_SYM7, 128, 1, 0, DEBUG>(tq, tk, tv, a, grid, cs);
   }
 }
 

@@ -1,6 +1,7 @@
-"""GPU parity of rotattn_fwd_int4 against the oracle's same-quantisation attention (O-quant):
-int32 S accumulators bit-exact, P codes within +-1 on <= 0.1 % of elements, O within 2e-2 max-abs and
-cosine >= 0.9999 (BASELINE.json north_star).  Everything goes through the C-ABI."""
+"""GPU parity of rotattn_fwd_int4 against the oracle's same-quantisation attention (O-quant): integer S and P~V accumulators
+bit-exact, P codes within +-1 on <= 0.1 % of elements, O within 2e-2 max-abs and cosine >= 0.9999 (BASELINE.json
+north_star); at full size the prologue is compared with the oracle from the fp16 inputs first.  Everything goes through
+the C-ABI."""
 import numpy as np
 import pytest
 
@@ -12,104 +13,57 @@ import __graft_entry__ as entry  # noqa: E402
 entry.build()
 from oracle import rotattn_oracle as orc  # noqa: E402
 from synth import video_qkv as syn  # noqa: E402
+import parity_helpers as ph  # noqa: E402
 
-O_ATOL = 2e-2       # north_star: max-abs 2e-2
-O_COS = 0.9999      # north_star: cosine >= 0.9999
-P_FRAC = 1e-3       # north_star: P codes differ by +-1 on <= 0.1 % of elements
-
-
-def _api():
-    from paper_2607_02584_b200 import api
-    return api
+F1 = [(128, orc.VSCALE_CHANNEL), (1, orc.VSCALE_GROUP), (128, orc.VSCALE_GROUP)]
 
 
-def _oracle_inputs(res, bi, h):
-    """codes/scales the kernel consumed (already proven bit-exact against the oracle's prologue in test_gpu_prologue)."""
-    qc = orc.unpack_nibbles(res['Q4'][bi, h].cpu().numpy())
-    kc = orc.unpack_nibbles(res['K4'][bi, h].cpu().numpy())
-    vc = orc.unpack_nibbles(res['V4'][bi, h].cpu().numpy())
-    return (qc, res['Qs'][bi, h].cpu().numpy(), kc, res['Ks'][bi, h].cpu().numpy(), vc, res['Vs'][bi, h].cpu().numpy())
-
-
-def _cos(a, b):
-    a, b = a.ravel().astype(np.float64), b.ravel().astype(np.float64)
-    return float(a @ b / (np.linalg.norm(a) * np.linalg.norm(b) + 1e-300))
-
-
-def _check_o(got, want):
-    assert np.isfinite(got).all()
-    assert np.abs(got - want).max() <= O_ATOL, np.abs(got - want).max()
-    assert _cos(got, want) >= O_COS, _cos(got, want)
-
-
-def _debug_tile(api, res, po, bh, q_tile):
-    p = res['p']
-    npad = -(-po.N // 128) * 128
-    S = torch.zeros((128, npad), dtype=torch.int32, device='cuda')
-    P = torch.zeros((128, npad), dtype=torch.uint8, device='cuda')
-    Ot = torch.zeros((128, po.D), dtype=torch.float16, device='cuda')
-    b = res['buffers']
-    api.rotattn_fwd_int4_debug(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, bh, q_tile, S, P, Ot, b.ws,
-                               api.WS_HAS_QK | api.WS_HAS_V)
-    torch.cuda.synchronize()
-    return S.cpu().numpy(), P.cpu().numpy(), Ot.float().cpu().numpy()
-
-
-def _check_tile(api, res, po, bi, h, q_tile, p_mode, p_norm):
-    N = po.N
-    rows = np.arange(q_tile * 128, min(N, (q_tile + 1) * 128))
-    qc, qs, kc, ks, vc, vs = _oracle_inputs(res, bi, h)
-    Ow, acc, codes = orc.o_quant(po, qc, qs, kc, ks, vc, vs, rows=rows, dump=True, p_mode=p_mode, p_norm=p_norm)
-    S, P, Ot = _debug_tile(api, res, po, bi * po.H + h, q_tile)
-    nr = len(rows)
-    assert np.array_equal(S[:nr, :N], acc), 'int32 QK^T accumulators differ'
-    diff = np.abs(P[:nr, :N].astype(np.int16) - codes)
-    assert diff.max() <= 1
-    assert (diff != 0).mean() <= P_FRAC, (diff != 0).mean()
-    assert np.all(P[:nr, N:] == 0)
-    _check_o(Ot[:nr], Ow)
-    full = res['O'][bi, h].float().cpu().numpy()[rows]
-    _check_o(full, Ow)
-
-
-@pytest.mark.parametrize('rot_mode', [orc.ROT_NONE, orc.ROT_INTERLEAVED, orc.ROT_HALF])
+@pytest.mark.parametrize('rot_mode', [orc.ROT_NONE, orc.ROT_INTERLEAVED, orc.ROT_HALF, orc.ROT_FULL])
 @pytest.mark.parametrize('p_mode', [orc.P_ASYM15, orc.P_SYM7])
 @pytest.mark.parametrize('p_norm', [orc.NORM_ROWBLOCK, orc.NORM_RUNNING])
 def test_tiny_all_modes(rot_mode, p_mode, p_norm):
-    api = _api()
     w = syn.TINY
     q, k, v = syn.gen_all(w)
-    res = api.run_int4(w, q, k, v, rot_mode=rot_mode, p_mode=p_mode, p_norm=p_norm)
-    torch.cuda.synchronize()
-    po = orc.Params(w.B, w.H, w.N, w.D, w.grid, w.pairs, rot_mode=rot_mode, p_mode=p_mode, p_norm=p_norm)
+    res, po, tab = ph.run_path(w, q, k, v, rot_mode=rot_mode, p_mode=p_mode, p_norm=p_norm)
     for h in range(w.H):
+        pq, vc, vs, _ = ph.check_prologue_head(po, tab, res, q[0, h], k[0, h], v[0, h], 0, h)
         for qt in range(2):
-            _check_tile(api, res, po, 0, h, qt, p_mode, p_norm)
+            ph.check_tile(res, po, 0, h, qt, inputs=(pq['q_codes'], pq['q_scale'], pq['k_codes'], pq['k_scale'], vc, vs))
 
 
 @pytest.mark.parametrize('base', [syn.WAN_1_3B, syn.HUNYUAN])
 def test_d128_ragged_multi_tile(base):
-    api = _api()
     w = syn.small_variant(base, (3, 9, 13), n_text=0 if base.n_text == 0 else 21, H=2)   # N = 351 / 372: 3 tiles, ragged
     q, k, v = syn.gen_all(w)
-    res = api.run_int4(w, q, k, v, rot_mode=orc.ROT_HALF)
-    torch.cuda.synchronize()
-    po = orc.Params(w.B, w.H, w.N, w.D, w.grid, w.pairs, rot_mode=orc.ROT_HALF)
+    res, po, tab = ph.run_path(w, q, k, v, rot_mode=orc.ROT_HALF)
     for h in range(w.H):
+        pq, vc, vs, _ = ph.check_prologue_head(po, tab, res, q[0, h], k[0, h], v[0, h], 0, h)
         for qt in range(3):
-            _check_tile(api, res, po, 0, h, qt, orc.P_ASYM15, orc.NORM_ROWBLOCK)
+            ph.check_tile(res, po, 0, h, qt, inputs=(pq['q_codes'], pq['q_scale'], pq['k_codes'], pq['k_scale'], vc, vs))
+
+
+@pytest.mark.parametrize('qk_group,v_scale', F1)
+@pytest.mark.parametrize('p_mode', [orc.P_ASYM15, orc.P_SYM7])
+def test_granularity_variants_tiny_and_ragged(qk_group, v_scale, p_mode):
+    """per-block Q/K scales and per-group V scales, same bounds, all rows of the tiny config plus a
+    ragged multi-tile D = 128 case with text tokens."""
+    for w in (syn.TINY, syn.small_variant(syn.HUNYUAN, (3, 9, 13), n_text=21, H=2)):
+        q, k, v = syn.gen_all(w)
+        res, po, tab = ph.run_path(w, q, k, v, rot_mode=orc.ROT_HALF, p_mode=p_mode, qk_group=qk_group, v_scale=v_scale)
+        for h in range(w.H):
+            pq, vc, vs, _ = ph.check_prologue_head(po, tab, res, q[0, h], k[0, h], v[0, h], 0, h)
+            for qt in range(-(-w.N // 128)):
+                ph.check_tile(res, po, 0, h, qt, inputs=(pq['q_codes'], pq['q_scale'], pq['k_codes'], pq['k_scale'], vc, vs))
 
 
 def test_fresh_workspace_unpack_path_and_head_sel():
     """fwd_int4 from the packed public buffers alone (ws_state = 0) and with a head subset."""
-    api = _api()
+    api = ph.api()
     w = syn.small_variant(syn.WAN_1_3B, (2, 9, 13), H=3)
     q, k, v = syn.gen_all(w)
-    res = api.run_int4(w, q, k, v, rot_mode=orc.ROT_HALF, use_ws=False)
-    torch.cuda.synchronize()
-    po = orc.Params(w.B, w.H, w.N, w.D, w.grid, w.pairs, rot_mode=orc.ROT_HALF)
-    qc, qs, kc, ks, vc, vs = _oracle_inputs(res, 0, 1)
-    _check_o(res['O'][0, 1].float().cpu().numpy(), orc.o_quant(po, qc, qs, kc, ks, vc, vs))
+    res, po, tab = ph.run_path(w, q, k, v, rot_mode=orc.ROT_HALF, use_ws=False)
+    qc, qs, kc, ks, vc, vs = ph.gpu_attention_inputs(res, 0, 1)
+    ph.check_o(res['O'][0, 1].float().cpu().numpy(), orc.o_quant(po, qc, qs, kc, ks, vc, vs))
     b = res['buffers']
     O2 = torch.full_like(b.O, 7.0)
     sel = torch.tensor([2, 0], dtype=torch.int32, device='cuda')
@@ -121,76 +75,165 @@ def test_fresh_workspace_unpack_path_and_head_sel():
 
 def test_diffuse_inputs_codes_cover_range():
     """No outliers (diffuse attention): the case where P-code rounding matters most."""
-    api = _api()
     w = syn.small_variant(syn.WAN_1_3B, (4, 8, 12), H=1)
     rng = np.random.default_rng(3)
     shape = (1, 1, w.N, w.D)
     q = (rng.standard_normal(shape) * 0.8).astype(np.float16)
     k = (rng.standard_normal(shape) * 0.8).astype(np.float16)
     v = rng.standard_normal(shape).astype(np.float16)
-    res = api.run_int4(w, q, k, v, rot_mode=orc.ROT_HALF)
-    torch.cuda.synchronize()
-    po = orc.Params(1, 1, w.N, w.D, w.grid, w.pairs, rot_mode=orc.ROT_HALF)
-    _check_tile(api, res, po, 0, 0, 1, orc.P_ASYM15, orc.NORM_ROWBLOCK)
-    _, P, _ = _debug_tile(api, res, po, 0, 0)
+    res, po, tab = ph.run_path(w, q, k, v, rot_mode=orc.ROT_HALF)
+    stats = []
+    ph.check_tile(res, po, 0, 0, 1, stats=stats)
+    print(f'diffuse tile: P-code mismatch rate {stats[0]:.2e} (bound {ph.P_FRAC:.0e})')
+    _, P, _, _ = ph.debug_tile(res, po, 0, 0)
     assert set(np.unique(P[:, :w.N])) == set(range(16))
+
+
+@pytest.mark.parametrize('rot_mode', [orc.ROT_NONE, orc.ROT_HALF])
+def test_smoothing_end_to_end(rot_mode):
+    """SURVEY 8f row f2 on inputs with a token-shared bias: prologue bit-exact, S / P / P~V / O within the usual bounds
+    (the per-key correction enters S in floating point, so integer S is still the codes' product)."""
+    w = syn.small_variant(syn.HUNYUAN, (3, 9, 13), n_text=21, H=2)
+    q, k, v = syn.gen_all(w)
+    rng = np.random.default_rng(10)
+    bias = (rng.standard_normal((1, 2, 1, w.D)) * 2).astype(np.float32)
+    q = (q.astype(np.float32) + bias).astype(np.float16)
+    k = (k.astype(np.float32) + bias).astype(np.float16)
+    v = (v.astype(np.float32) + bias).astype(np.float16)
+    res, po, tab = ph.run_path(w, q, k, v, rot_mode=rot_mode, smooth=1)
+    for h in range(w.H):
+        pq, vc, vs, means = ph.check_prologue_head(po, tab, res, q[0, h], k[0, h], v[0, h], 0, h)
+        for qt in range(3):
+            ph.check_tile(res, po, 0, h, qt, inputs=(pq['q_codes'], pq['q_scale'], pq['k_codes'], pq['k_scale'], vc, vs),
+                          k_corr=pq['k_corr'], v_mean=means[2])
+
+
+def _crafted(N, D, qc, kc, vc, qs, ks, vs, p_mode=orc.P_ASYM15):
+    """Run fwd_int4 on hand-made codes (packed public buffers, fresh workspace): returns (res, po)."""
+    api = ph.api()
+    w = syn.small_variant(syn.WAN_1_3B if D == 128 else syn.TINY, (1, 1, N), H=1)
+    p = api.params_for(w, p_mode=p_mode)
+    po = ph.oracle_params(w, 1, p_mode=p_mode)
+    b = api.Buffers(p)
+    b.Q4.copy_(torch.from_numpy(orc.pack_nibbles(qc))[None, None])
+    b.K4.copy_(torch.from_numpy(orc.pack_nibbles(kc))[None, None])
+    b.V4.copy_(torch.from_numpy(orc.pack_nibbles(vc))[None, None])
+    b.Qs.copy_(torch.from_numpy(qs)[None, None]); b.Ks.copy_(torch.from_numpy(ks)[None, None]); b.Vs.copy_(torch.from_numpy(vs)[None, None])
+    api.rotattn_fwd_int4(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, b.O, b.ws, 0)
+    torch.cuda.synchronize()
+    return dict(p=p, buffers=b, Q4=b.Q4, K4=b.K4, V4=b.V4, Qs=b.Qs, Ks=b.Ks, Vs=b.Vs, O=b.O), po
+
+
+@pytest.mark.parametrize('unit', [1, -1])
+def test_adversarial_integer_exactness_in_the_attention_kernel(unit):
+    """Maximum dynamic range inside fwd_int4 itself: S accumulators at +-(49 * 127) receiving one +-1-unit product at
+    every position of the contraction, and P~V accumulators at 15 * 7 * 127 receiving unit products (flat softmax: every
+    P code is 15) - both dumped and compared bit for bit (the E4M3 path is admissible only if exact)."""
+    N, D = 384, 128
+    qc = np.full((N, D), 7, dtype=np.int8)
+    kc = np.full((N, D), 7, dtype=np.int8)
+    idx = np.arange(N)
+    qc[idx, idx % D] = 1
+    kc[idx, idx % D] = unit                       # key j: unit factor at position j mod D -> meets q's unit when i = j mod D
+    kc[1::2] *= -1                                # every other key negative: S = -/+ 6223 +- 1
+    vc = np.full((N, D), 7, dtype=np.int8)
+    vc[idx, idx % D] = unit                       # one unit code per key, at channel j mod D
+    vc[:, 1::2] *= -1
+    qs = np.full(N, 1e-4, dtype=np.float32)       # tiny scales: s ~ 0, P^ ~ 1, every code saturates at 15
+    ks = np.full(N, 1e-4, dtype=np.float32)
+    vs = np.ones((3, D), dtype=np.float32)
+    res, po = _crafted(N, D, qc, kc, vc, qs, ks, vs)
+    for qt in range(3):
+        ph.check_tile(res, po, 0, 0, qt)
+    S, P, PV, _ = ph.debug_tile(res, po, 0, 0)
+    assert np.abs(S).max() >= 49 * 127 - 1 and set(np.unique(P[:, :N])) == {15}
+    assert np.abs(PV).max() >= 15 * (7 * 127 - 1)
+
+
+def test_random_codes_full_range_through_the_attention_kernel():
+    """Random codes over the full ranges with random scales: S, P~V bit-exact, P codes and O within bounds."""
+    rng = np.random.default_rng(23)
+    N, D = 640, 128
+    qc = rng.integers(-7, 8, (N, D)).astype(np.int8)
+    kc = rng.integers(-7, 8, (N, D)).astype(np.int8)
+    vc = rng.integers(-7, 8, (N, D)).astype(np.int8)
+    qs = rng.uniform(0.02, 0.08, N).astype(np.float32)
+    ks = rng.uniform(0.02, 0.08, N).astype(np.float32)
+    vs = rng.uniform(0.1, 0.5, (5, D)).astype(np.float32)
+    res, po = _crafted(N, D, qc, kc, vc, qs, ks, vs)
+    for qt in range(5):
+        ph.check_tile(res, po, 0, 0, qt)
 
 
 def test_full_size_wan13b_row_sample():
     """BASELINE.json configs[1] at full size, the launch configuration bench.py times; oracle on a seeded row sample."""
-    api = _api()
     w = syn.WAN_1_3B
     q, k, v = syn.gen_all(w)
-    res = api.run_int4(w, q, k, v, rot_mode=orc.ROT_HALF)
-    torch.cuda.synchronize()
-    po = orc.Params(w.B, w.H, w.N, w.D, w.grid, w.pairs, rot_mode=orc.ROT_HALF)
+    res, po, tab = ph.run_path(w, q, k, v, rot_mode=orc.ROT_HALF)
     for h in (0, 5):
+        pq, vc, vs, _ = ph.check_prologue_head(po, tab, res, q[0, h], k[0, h], v[0, h], 0, h)
+        inputs = (pq['q_codes'], pq['q_scale'], pq['k_codes'], pq['k_scale'], vc, vs)
         rows = syn.sample_rows(w, n_tiles=3, head=h)
         tiles = sorted(set((rows // 128).tolist()))
-        _check_tile(api, res, po, 0, h, tiles[-1], orc.P_ASYM15, orc.NORM_ROWBLOCK)      # ragged last tile, with dumps
-        qc, qs, kc, ks, vc, vs = _oracle_inputs(res, 0, h)
-        Ow = orc.o_quant(po, qc, qs, kc, ks, vc, vs, rows=rows)
-        _check_o(res['O'][0, h].float().cpu().numpy()[rows], Ow)
+        ph.check_tile(res, po, 0, h, tiles[-1], inputs=inputs)      # ragged last tile, with dumps
+        ph.check_o(res['O'][0, h].float().cpu().numpy()[rows], orc.o_quant(po, *inputs, rows=rows))
 
 
-def _full_size_case(w, heads, p_mode=orc.P_ASYM15, rot_mode=orc.ROT_HALF, n_tiles=3):
-    """Full N and D of a BASELINE.json config on a seeded subset of its heads (heads are independent units):
-    prologue codes bit-exact on the sampled rows' inputs, S/P dumps on the ragged last tile, O on a seeded row sample."""
-    api = _api()
-    q, k, v = syn.gen_all(w, heads=heads)
-    res = api.run_int4(w, q, k, v, rot_mode=rot_mode, p_mode=p_mode)
-    torch.cuda.synchronize()
-    po = orc.Params(w.B, len(heads), w.N, w.D, w.grid, w.pairs, rot_mode=rot_mode, p_mode=p_mode)
-    for i, h in enumerate(heads):
+def _full_size_case(w, heads, n_tiles=3, **modes):
+    """Full N, D and ALL heads of a BASELINE.json config in one launch (the grid and workspace sizes bench.py uses).  For
+    the sampled heads: Q/K/V codes, scales and operand bytes against the oracle from the fp16 inputs (bit-exact), S / P /
+    P~V dumps on the ragged last tile, O on a seeded row sample."""
+    q, k, v = syn.gen_all(w)
+    res, po, tab = ph.run_path(w, q, k, v, **modes)
+    assert res['O'].shape[1] == w.H
+    for h in heads:
+        pq, vc, vs, _ = ph.check_prologue_head(po, tab, res, q[0, h], k[0, h], v[0, h], 0, h)
+        inputs = (pq['q_codes'], pq['q_scale'], pq['k_codes'], pq['k_scale'], vc, vs)
         rows = syn.sample_rows(w, n_tiles=n_tiles, head=h)
         tiles = sorted(set((rows // 128).tolist()))
-        _check_tile(api, res, po, 0, i, tiles[-1], p_mode, orc.NORM_ROWBLOCK)
-        qc, qs, kc, ks, vc, vs = _oracle_inputs(res, 0, i)
-        Ow = orc.o_quant(po, qc, qs, kc, ks, vc, vs, rows=rows, p_mode=p_mode)
-        _check_o(res['O'][0, i].float().cpu().numpy()[rows], Ow)
-    return res, po
+        ph.check_tile(res, po, 0, h, tiles[-1], inputs=inputs)
+        ph.check_o(res['O'][0, h].float().cpu().numpy()[rows], orc.o_quant(po, *inputs, rows=rows))
+    # no head was left unwritten / non-finite
+    assert bool(torch.isfinite(res['O'].float()).all())
+    del res
+    torch.cuda.empty_cache()
 
 
-def test_full_size_wan14b_row_sample():
-    """BASELINE.json configs[2] (N = 75600, per-head outlier pairs with magnitudes U(5,25)), heads 0 and 17."""
-    _full_size_case(syn.WAN_14B, [0, 17])
+NAIVE = dict(rot_mode=orc.ROT_NONE, p_mode=orc.P_SYM7)       # north_star: naive symmetric-INT4, no-rotation baseline
 
 
-def test_full_size_hunyuan_row_sample_with_text_tokens():
-    """BASELINE.json configs[3] (N = 118800 video + 256 text tokens without RoPE, split 8/28/28), heads 3 and 11."""
-    _full_size_case(syn.HUNYUAN, [3, 11])
+def test_full_size_wan14b_all_heads():
+    """BASELINE.json configs[2] (H = 40, N = 75600, per-head outlier pairs with magnitudes U(5,25)); heads 0 and 39 checked."""
+    _full_size_case(syn.WAN_14B, [0, 39], rot_mode=orc.ROT_HALF)
 
 
-def test_sweep_largest_n_and_naive_mode():
-    """BASELINE.json configs[4]: the largest sweep point (N = 131072) in the headline mode, and the naive
-    symmetric-INT4 / no-rotation baseline (NONE + SYM7) at N = 16384."""
-    _full_size_case(syn.SWEEP[4], [1], n_tiles=2)
-    _full_size_case(syn.SWEEP[1], [2], p_mode=orc.P_SYM7, rot_mode=orc.ROT_NONE, n_tiles=2)
+def test_full_size_wan14b_naive_mode():
+    _full_size_case(syn.WAN_14B, [17], n_tiles=2, **NAIVE)
+
+
+def test_full_size_hunyuan_all_heads_with_text_tokens():
+    """BASELINE.json configs[3] (H = 24, N = 118800 video + 256 text tokens without RoPE, split 8/28/28); heads 3 and 23."""
+    _full_size_case(syn.HUNYUAN, [3, 23], rot_mode=orc.ROT_HALF)
+
+
+def test_full_size_hunyuan_naive_mode():
+    _full_size_case(syn.HUNYUAN, [11], n_tiles=2, **NAIVE)
+
+
+@pytest.mark.parametrize('idx', [0, 1, 2, 3, 4])
+def test_sweep_points_all_heads(idx):
+    """BASELINE.json configs[4]: every sweep point (N = 4096 .. 131072, H = 24, split 8/28/28) in the headline mode."""
+    _full_size_case(syn.SWEEP[idx], [1, 22] if idx < 3 else [1], n_tiles=2, rot_mode=orc.ROT_HALF)
+
+
+def test_sweep_naive_mode_and_granularity_variants_at_16384():
+    _full_size_case(syn.SWEEP[1], [2], n_tiles=2, **NAIVE)
+    _full_size_case(syn.SWEEP[1], [5], n_tiles=2, rot_mode=orc.ROT_HALF, qk_group=128, v_scale=orc.VSCALE_GROUP)
 
 
 def test_mixed_precision_step_head_split():
     """configs[4] schedule step: FP16 fallback on a head subset, INT4 on the rest, both through head_sel into one O."""
-    api = _api()
+    api = ph.api()
     w = syn.small_variant(syn.SWEEP[0], (4, 16, 16), H=5)          # N = 1024
     q, k, v = syn.gen_all(w)
     res = api.run_int4(w, q, k, v, rot_mode=orc.ROT_HALF, want_fp16=True)
@@ -213,28 +256,23 @@ def test_mixed_precision_step_head_split():
 @pytest.mark.parametrize('p_mode', [orc.P_ASYM15, orc.P_SYM7])
 def test_d128_running_normaliser_ragged(p_mode):
     """p_norm = RUNNING (the other reading of Eq.12's normaliser) at D = 128 over several ragged tiles."""
-    api = _api()
     w = syn.small_variant(syn.HUNYUAN, (3, 9, 13), n_text=21, H=2)
     q, k, v = syn.gen_all(w)
-    res = api.run_int4(w, q, k, v, rot_mode=orc.ROT_HALF, p_mode=p_mode, p_norm=orc.NORM_RUNNING)
-    torch.cuda.synchronize()
-    po = orc.Params(w.B, w.H, w.N, w.D, w.grid, w.pairs, rot_mode=orc.ROT_HALF, p_mode=p_mode, p_norm=orc.NORM_RUNNING)
+    res, po, tab = ph.run_path(w, q, k, v, rot_mode=orc.ROT_HALF, p_mode=p_mode, p_norm=orc.NORM_RUNNING)
     for h in range(w.H):
         for qt in range(3):
-            _check_tile(api, res, po, 0, h, qt, p_mode, orc.NORM_RUNNING)
+            ph.check_tile(res, po, 0, h, qt)
 
 
 def test_batch_of_two_and_d64_many_tiles():
     """B = 2 (unit index = b * H + h) and D = 64 over 9 KV blocks with a ragged tail."""
-    api = _api()
     from dataclasses import replace
     w = replace(syn.small_variant(syn.TINY, (4, 16, 17), H=2), B=2)      # N = 1088 = 8 * 128 + 64
     q, k, v = syn.gen_all(w)
-    res = api.run_int4(w, q, k, v, rot_mode=orc.ROT_INTERLEAVED)
-    torch.cuda.synchronize()
-    po = orc.Params(w.B, w.H, w.N, w.D, w.grid, w.pairs, rot_mode=orc.ROT_INTERLEAVED)
+    res, po, tab = ph.run_path(w, q, k, v, rot_mode=orc.ROT_INTERLEAVED)
     for bi in range(2):
         for h in range(2):
-            qc, qs, kc, ks, vc, vs = _oracle_inputs(res, bi, h)
-            _check_o(res['O'][bi, h].float().cpu().numpy(), orc.o_quant(po, qc, qs, kc, ks, vc, vs))
-    _check_tile(api, res, po, 1, 1, 8, orc.P_ASYM15, orc.NORM_ROWBLOCK)
+            pq, vc, vs, _ = ph.check_prologue_head(po, tab, res, q[bi, h], k[bi, h], v[bi, h], bi, h)
+            ph.check_o(res['O'][bi, h].float().cpu().numpy(),
+                       orc.o_quant(po, pq['q_codes'], pq['q_scale'], pq['k_codes'], pq['k_scale'], vc, vs))
+    ph.check_tile(res, po, 1, 1, 8)

@@ -227,6 +227,104 @@ def test_incoherence_definition():
     assert np.allclose(orc.incoherence(x), [1.0, 4.0])              # mean (2,2): max |x-mean|
 
 
+# ---------------------------------------------------------------- "Full" rotation baseline (L208, Eq.13)
+@pytest.mark.parametrize('D', [64, 128])
+def test_full_rotation_butterfly_is_the_dense_hadamard(D):
+    """The fp32 butterfly equals y H_D / sqrt(D) with the library Sylvester matrix; H is symmetric and orthogonal, so
+    applying it twice returns y; a unit vector e_c maps to column c of H (catches a wrong stride order or sign)."""
+    rng = np.random.default_rng(30)
+    y = (rng.standard_normal((37, D)) * 3).astype(np.float32)
+    H = scipy_hadamard(D).astype(np.float64) / math.sqrt(D)
+    got = orc.fwht_fp32(y)
+    want = y.astype(np.float64) @ H
+    assert got.dtype == np.float32 and np.abs(got - want).max() <= 8 * 2.0 ** -24 * np.abs(want).max() * math.log2(D)
+    assert np.abs(orc.fwht_fp32(got) - y).max() <= 1e-5 * np.abs(y).max()
+    e = np.eye(D, dtype=np.float32)
+    assert np.allclose(orc.fwht_fp32(e), H, atol=1e-7)
+    p = orc.Params(1, 1, 37, D, (1, 1, 37), (D // 2 - 20, 10, 10), rot_mode=orc.ROT_FULL)
+    assert np.allclose(orc.dense_rotation(p, orc.ROT_FULL), H, atol=1e-15)
+
+
+def test_full_rotation_keeps_qk_and_flattens_incoherence():
+    """Eq.5 with R = H_D (orthogonal): QK^T unchanged; on the tiny workload the Full rotation spreads the outlier pairs
+    over all channels, so max Psi drops at least as much as with Half (L141, L208)."""
+    p = _params(orc.ROT_FULL, N=N0 + 3)
+    rng = np.random.default_rng(31)
+    q, k = rng.standard_normal((p.N, p.D)), rng.standard_normal((p.N, p.D))
+    S0 = orc.rope_fp64(p, q) @ orc.rope_fp64(p, k).T
+    S1 = orc.rope_fp64(p, q, orc.ROT_FULL) @ orc.rope_fp64(p, k, orc.ROT_FULL).T
+    assert np.abs(S0 - S1).max() <= 1e-9 * np.abs(S0).max()
+    x16 = (rng.standard_normal((p.N, p.D)) * 2).astype(np.float16)
+    y32 = orc.apply_rope_rot(p, x16, orc.coef_table(p))
+    y64 = orc.rope_fp64(p, x16.astype(np.float64), orc.ROT_FULL)
+    assert np.abs(y32 - y64).max() <= 4e-6 * np.abs(y64).max()
+    w = syn.TINY
+    q16, _, _ = syn.gen_head(w, 0, 0)
+    psi = {}
+    for mode in (orc.ROT_NONE, orc.ROT_HALF, orc.ROT_FULL):
+        pm = orc.Params(1, 1, w.N, w.D, w.grid, w.pairs, rot_mode=mode)
+        psi[mode] = orc.incoherence(orc.apply_rope_rot(pm, q16, orc.coef_table(pm))).max()
+    assert psi[orc.ROT_FULL] < psi[orc.ROT_HALF] < psi[orc.ROT_NONE]
+
+
+# ---------------------------------------------------------------- smoothing (L90, L40, L52)
+def test_column_mean_fixed_point_is_order_independent_and_close_to_the_mean():
+    rng = np.random.default_rng(32)
+    x = (rng.standard_normal((1000, 16)) * np.exp(rng.standard_normal((1, 16)) * 2) + 3.0).astype(np.float32)
+    m = orc.column_mean_fixed(x, orc.FIX_QK)
+    assert m.dtype == np.float32
+    assert np.array_equal(m, orc.column_mean_fixed(x[rng.permutation(1000)], orc.FIX_QK))        # any order of summation
+    assert np.abs(m - x.astype(np.float64).mean(axis=0)).max() <= 2.0 ** -21 + 1e-7 * np.abs(x).max()
+    v = rng.standard_normal((513, 8)).astype(np.float16)
+    mv = orc.column_mean_fixed(v.astype(np.float32), orc.FIX_V)
+    assert np.array_equal(mv, v.astype(np.float64).mean(axis=0).astype(np.float32))            # fp16 data: the sum is exact
+    # hand-written case: (1 + 2 + 6) / 3 = 3 and (0.5 - 0.25 + 0.125) / 3 = 0.125
+    t = np.array([[1.0, 0.5], [2.0, -0.25], [6.0, 0.125]], dtype=np.float32)
+    assert np.array_equal(orc.column_mean_fixed(t, orc.FIX_QK), np.array([3.0, 0.125], dtype=np.float32))
+
+
+def test_smoothing_shifts_are_exact_without_quantisers():
+    """The three identities behind the smoothing path, in fp64 on real-valued tensors (no quantiser): K - mean K leaves
+    softmax(QK^T) unchanged; (Q - mean Q) K'^T + 1 (mean Q . K'_j) = Q K'^T; softmax(.)(V - mean V) + mean V = softmax(.) V.
+    Checked through o_quant(quantize=False) with the k_corr / v_mean arguments, against the plain definition."""
+    rng = np.random.default_rng(33)
+    N, D = 300, 32
+    q = rng.standard_normal((N, D)) + rng.standard_normal((1, D)) * 2      # token-shared biases
+    k = rng.standard_normal((N, D)) + rng.standard_normal((1, D)) * 2
+    v = rng.standard_normal((N, D)) + rng.standard_normal((1, D)) * 3
+    want = orc.o_exact(q, k, v)
+    mq, mk, mv = q.mean(0), k.mean(0), v.mean(0)
+    qp, kp, vp = q - mq, k - mk, v - mv
+    assert np.allclose(orc.o_exact(q, kp, v), want, atol=1e-12)                       # K shift alone
+    p = orc.Params(1, 1, N, D, (1, 1, N), (4, 4, 8))
+    ones = np.ones(N, dtype=np.float32)
+    # "codes" = the real values themselves (quantisers off), unit scales
+    O = orc.o_quant(p, qp, ones, kp, ones, vp, np.ones((3, D), dtype=np.float32), quantize=False, k_corr=kp @ mq, v_mean=mv)
+    assert np.allclose(O, want, atol=1e-11)
+    O_nocorr = orc.o_quant(p, qp, ones, kp, ones, vp, np.ones((3, D), dtype=np.float32), quantize=False, v_mean=mv)
+    assert not np.allclose(O_nocorr, want, atol=1e-3)                                 # dropping the rank-1 term is visible
+
+
+def test_smoothing_helps_on_token_shared_bias():
+    """L90 / L40: with a bias shared by all tokens the smoothed INT4 path is closer to exact attention."""
+    rng = np.random.default_rng(34)
+    N, D = 512, 64
+    bias = np.zeros((1, D)); bias[0, rng.choice(D, 6, replace=False)] = rng.uniform(4, 8, 6) * rng.choice([-1, 1], 6)
+    q16 = (rng.standard_normal((N, D)) * 0.7 + bias).astype(np.float16)
+    k16 = (rng.standard_normal((N, D)) * 0.7 + bias).astype(np.float16)
+    v16 = (rng.standard_normal((N, D)) + bias * 0.5).astype(np.float16)
+    errs = {}
+    for sm in (0, 1):
+        p = orc.Params(1, 1, N, D, (8, 8, 8), (12, 10, 10), rot_mode=orc.ROT_NONE, smooth=sm)
+        O, pq, _ = orc.int4_attention_head(p, q16, k16, v16)
+        ex = orc.o_exact(orc.rope_fp64(p, q16.astype(np.float64)), orc.rope_fp64(p, k16.astype(np.float64)), v16.astype(np.float64))
+        errs[sm] = np.abs(O - ex).sum() / np.abs(ex).sum()
+        if sm:
+            mq, mk, mv = pq['means']
+            assert np.abs(pq['q_y'].mean(0)).max() < 1e-3 and np.abs(pq['k_y'].mean(0)).max() < 1e-3
+    assert errs[1] < 0.8 * errs[0], errs
+
+
 # ---------------------------------------------------------------- quantisers (L190)
 def test_quantiser_properties():
     rng = np.random.default_rng(7)
@@ -263,6 +361,38 @@ def test_v_group_quantiser():
         err = np.abs(v[sl].astype(np.float32) - codes[sl] * scales[g][None, :])
         assert np.all(err <= scales[g][None, :] / 2 * (1 + 1e-6))
         assert np.all(np.abs(codes[sl]).max(axis=0) == 7)
+
+
+def test_v_scalar_group_quantiser():
+    """one V scale per 128-token group (amax over tokens and channels)."""
+    rng = np.random.default_rng(35)
+    v = (rng.standard_normal((300, 16)) * np.array([1, 4] * 8)).astype(np.float16)
+    codes, scales = orc.quant_v(v, 128, orc.VSCALE_GROUP)
+    assert scales.shape == (3,)
+    for g in range(3):
+        sl = slice(128 * g, min(300, 128 * (g + 1)))
+        x = v[sl].astype(np.float32)
+        assert np.isclose(scales[g], np.abs(x).max() / 7, rtol=1e-6)
+        assert np.all(np.abs(x - codes[sl] * scales[g]) <= scales[g] / 2 * (1 + 1e-6))
+        assert np.abs(codes[sl]).max() == 7 and codes[sl].min() >= -7
+    c2, s2 = orc.quant_v((codes * scales.repeat(128)[:300, None]).astype(np.float16), 128, orc.VSCALE_GROUP)
+    # o_quant accepts both scale shapes: a per-group scalar equals the same value repeated over the channels
+    p, qc, qs, kc, ks, vc, vs = _tiny_problem()
+    vg = vs[:, 0].copy()
+    O1 = orc.o_quant(p, qc, qs, kc, ks, vc, vg)
+    O2 = orc.o_quant(p, qc, qs, kc, ks, vc, np.repeat(vg[:, None], vc.shape[1], axis=1))
+    assert np.array_equal(O1, O2)
+
+
+def test_qk_block_scales_in_o_quant():
+    """qk_group = 128 (north_star "per-block scales"): o_quant picks scale[n // 128]; equals per-token scales repeated."""
+    p, qc, qs, kc, ks, vc, vs = _tiny_problem()
+    import dataclasses
+    pg = dataclasses.replace(p, qk_group=128)
+    qg, kg = qs[::128].copy(), ks[::128].copy()
+    O1 = orc.o_quant(pg, qc, qg, kc, kg, vc, vs)
+    O2 = orc.o_quant(p, qc, np.repeat(qg, 128)[:300], kc, np.repeat(kg, 128)[:300], vc, vs)
+    assert np.array_equal(O1, O2)
 
 
 def test_pack_unpack_all_nibble_pairs():
