@@ -7,7 +7,8 @@ rotattn_fwd_int4, all through the C-ABI.  `value` = effective TOPS = 4*B*H*N^2*D
 resident in HBM; `e2e` = the same with HOST (pinned) Q,K,V copied in and O copied out inside the timed region.
 The FP16 fallback kernel is timed beside it (speed-up denominator) but is not part of the step.
 N > 1 (torchrun): every rank runs the full workload on its own GPU (independent (b,h) units, no collective);
-value = total ops of all ranks / max-over-ranks time ("weak").
+value = total ops of all ranks / max-over-ranks time ("weak").  `--head-shard` instead splits the heads of ONE workload
+over the ranks with paper_2607_02584_b200.dist.shard_heads ("strong").
 `--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload.
 """
 from __future__ import annotations
@@ -15,6 +16,7 @@ from __future__ import annotations
 import argparse
 import json
 import os
+import platform
 import subprocess
 import sys
 import threading
@@ -27,6 +29,7 @@ sys.path.insert(0, ROOT)
 
 METRIC = 'INT4 attn fwd effective TOPS (4*B*H*N^2*D ops per call; N=32760,H=12,D=128); ms/call in ms_per_step'
 WORKLOAD = 'wan1.3b-480p'
+DTYPE = 'INT4 codes carried as exact E4M3 bytes (code * 2^-9) on tcgen05 kind::f8f6f4, fp32 accumulators holding the integers; fp32 softmax'
 
 
 def _peaks():
@@ -39,44 +42,78 @@ def _peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons DURING the timed region."""
+    """nvidia-smi clocks / throttle reasons; started BEFORE the warm-up (its first row takes a few hundred ms), marked at
+    the start and end of the timed region so that only samples taken under load are summarised."""
     Q = 'clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,' \
-        'clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap'
+        'clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap,power.draw'
 
     def __init__(self, index):
-        self.index, self.rows, self.proc = index, [], None
+        self.index, self.rows, self.proc, self.t0, self.t1 = index, [], None, None, None
 
     def start(self):
         try:
             self.proc = subprocess.Popen(['nvidia-smi', '-i', str(self.index), f'--query-gpu={self.Q}',
-                                          '--format=csv,noheader,nounits', '-lms', '20'],
+                                          '--format=csv,noheader,nounits', '-lms', '10'],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
+            t = time.time()
+            while not self.rows and time.time() - t < 3.0:
+                time.sleep(0.01)
         except Exception:
             self.proc = None
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append([x.strip() for x in line.split(',')])
+            self.rows.append((time.time(), [x.strip() for x in line.split(',')]))
+
+    def mark(self, begin):
+        if begin:
+            self.t0 = time.time()
+        else:
+            self.t1 = time.time()
 
     def stop(self):
         if not self.proc:
-            return {'sm_mhz': None, 'sm_max_mhz': None, 'reasons': ['nvidia-smi unavailable']}
+            return {'sm_mhz': None, 'sm_max_mhz': None, 'reasons': ['nvidia-smi unavailable'], 'samples': 0}
+        time.sleep(0.05)
         self.proc.terminate()
         try:
             self.proc.wait(timeout=2)
         except Exception:
             self.proc.kill()
-        sm = [float(r[0]) for r in self.rows if len(r) >= 6 and r[0].replace('.', '').isdigit()]
-        mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace('.', '').isdigit()]
         names = ['hw_slowdown', 'hw_thermal_slowdown', 'sw_thermal_slowdown', 'sw_power_cap']
-        reasons = [n for i, n in enumerate(names) if any(len(r) >= 6 and r[2 + i].lower().startswith('active') for r in self.rows)]
-        return {'sm_mhz': float(np.median(sm)) if sm else None, 'sm_max_mhz': max(mx) if mx else None, 'reasons': reasons,
-                'samples': len(sm)}
+
+        def summarise(rows):
+            ok = [r for _, r in rows if len(r) >= 7 and r[0].replace('.', '').isdigit()]
+            sm = [float(r[0]) for r in ok]
+            counts = {n: sum(1 for r in ok if r[2 + i].lower().startswith('active')) for i, n in enumerate(names)}
+            return ok, sm, counts
+        load = [(t, r) for t, r in self.rows if self.t0 is not None and self.t0 - 0.02 <= t <= (self.t1 or 1e30) + 0.02]
+        ok, sm, counts = summarise(load)
+        allok, allsm, _ = summarise(self.rows)
+        mx = [float(r[1]) for r in allok]
+        out = {'sm_mhz': float(np.median(sm)) if sm else (float(np.median(allsm)) if allsm else None),
+               'sm_mhz_min': min(sm) if sm else None, 'sm_max_mhz': max(mx) if mx else None,
+               'reasons': [n for n in names if counts[n]], 'reason_samples': counts,
+               'samples': len(sm), 'samples_total': len(allsm),
+               'power_w_max': max((float(r[6]) for r in ok if r[6].replace('.', '').isdigit()), default=None)}
+        if len(sm) < 20:
+            out['note'] = 'fewer than 20 samples inside the timed region: throttle reasons may be under-sampled'
+        return out
 
 
-def cpu_oracle_sample(n_rows=1024, threads=None):
+def _cpu_model():
+    try:
+        for line in open('/proc/cpuinfo'):
+            if line.startswith('model name'):
+                return line.split(':', 1)[1].strip()
+    except OSError:
+        pass
+    return platform.processor() or 'unknown'
+
+
+def cpu_oracle_sample(n_rows=1024):
     """Time the oracle as it stands on a bounded sample of the workload: one head's full prologue
     (RoPE + Half rotation + INT4 Q/K, V quantiser on all N tokens) + quantised attention for n_rows query rows
     against all N keys.  Returns (seconds, ops) with ops = 4*rows*N*D."""
@@ -92,6 +129,25 @@ def cpu_oracle_sample(n_rows=1024, threads=None):
     return dt, 4.0 * len(rows) * w.N * w.D, len(rows)
 
 
+def cpu_baseline_block(n_rows, total_rows):
+    """cpu_baseline: the oracle on all host cores, a second line pinned to one BLAS thread (subprocess, so that the
+    thread count is really applied), the CPU model and the labelled extrapolation to the full call."""
+    dt, cops, nrows = cpu_oracle_sample(n_rows)
+    one = None
+    try:
+        env = dict(os.environ, OMP_NUM_THREADS='1', OPENBLAS_NUM_THREADS='1', MKL_NUM_THREADS='1')
+        r = subprocess.run([sys.executable, os.path.abspath(__file__), '--impl', 'oracle-sample', '--rows', '256'],
+                           env=env, capture_output=True, text=True, timeout=600)
+        one = json.loads(r.stdout.strip().splitlines()[-1])
+    except Exception as e:          # the one-thread line is informative only
+        one = {'error': str(e)[:200]}
+    w_desc = f'{WORKLOAD}: 1 head, full prologue on all N tokens + O-quant for {nrows} query rows x all keys'
+    return {'value': cops / dt / 1e12, 'unit': 'TOPS', 'cores': os.cpu_count(), 'kind': 'oracle', 'seconds': dt, 'sample': w_desc,
+            'cpu_model': _cpu_model(), 'one_thread': one,
+            'extrapolated_full_call_seconds': dt * total_rows / nrows,
+            'extrapolation': f'measured sample time x (B*H*N = {total_rows} query rows) / ({nrows} sampled rows): an extrapolation, not a measurement'}
+
+
 def _time_ms(torch, fn, iters, warm=1):
     for _ in range(warm):
         fn()
@@ -105,44 +161,118 @@ def _time_ms(torch, fn, iters, warm=1):
     return e0.elapsed_time(e1) / iters
 
 
-def quality_report(api, syn, torch, w, Q, K, V, b, coef):
-    """Quality of the INT4 path against exact attention, next to the naive symmetric-INT4 / no-rotation baseline
-    (north_star).  The exact reference here is the library's own FP16 kernel on the same inputs (within 2e-3 of fp64
-    attention, tests/test_gpu_fwd_fp16.py); everything runs on the GPU, heads 0..3 of the bench workload."""
-    def metrics(o, ref):
-        o, ref = o.double().flatten(), ref.double().flatten()
-        return {'cosine': float((o @ ref) / (o.norm() * ref.norm())), 'rel_l1': float((o - ref).abs().sum() / ref.abs().sum())}
-    H4 = min(4, w.H)
+def measured_8bit_peaks(api, torch):
+    """Dense 8-bit tensor rates measured in this run: the library's own tcgen05 GEMM probe (kind::i8 and kind::f8f6f4, the
+    path the attention kernel uses) and torch._int_mm (cuBLASLt) at 8192^3."""
     out = {}
-    sl = lambda t: t[:, :H4].contiguous()
-    Qh, Kh, Vh = sl(Q), sl(K), sl(V)
-    ref = None
-    for name, rot, pm in (('half_asym15', api.ROT_HALF, api.P_ASYM15), ('interleaved_asym15', api.ROT_INTERLEAVED, api.P_ASYM15),
-                          ('none_asym15', api.ROT_NONE, api.P_ASYM15), ('naive_none_sym7', api.ROT_NONE, api.P_SYM7)):
-        p = api.params_for(w, rot, pm, H=H4)
-        cf = torch.from_numpy(api.rotattn_build_tables(p)).cuda()
-        bb = api.Buffers(p, want_fp16=ref is None)
-        api.rotattn_prepare_qk(p, cf, None, Qh, Kh, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.Q16, bb.K16, bb.ws)
-        api.rotattn_quant_v(p, Vh, bb.V4, bb.Vs, bb.ws)
-        api.rotattn_fwd_int4(p, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.V4, bb.Vs, bb.O, bb.ws, api.WS_HAS_QK | api.WS_HAS_V)
-        if ref is None:
-            api.rotattn_fwd_fp16(p, bb.Q16, bb.K16, Vh, bb.O16, bb.ws16)
-            ref = bb.O16.clone()
-        torch.cuda.synchronize()
-        out[name] = metrics(bb.O, ref)
-    out['note'] = 'synthetic outlier inputs (stand-ins for Wan2.2 activations); paper reports video-level metrics only (Table 1)'
+    M = N = K = 8192
+    ops = 2.0 * M * N * K
+    a8 = torch.randint(-7, 8, (M, K), device='cuda', dtype=torch.int8)
+    b8 = torch.randint(-7, 8, (N, K), device='cuda', dtype=torch.int8)
+    c32 = torch.empty((M, N), device='cuda', dtype=torch.int32)
+    cf = torch.empty((M, N), device='cuda', dtype=torch.float32)
+    au, bu = a8.view(torch.uint8), b8.view(torch.uint8)
+    try:
+        out['probe_kind_i8_tops'] = ops / _time_ms(torch, lambda: api.rotattn_probe_gemm8(M, N, K, a8, b8, c32, 0), 5, 2) / 1e9
+        out['probe_kind_f8f6f4_tops'] = ops / _time_ms(torch, lambda: api.rotattn_probe_gemm8(M, N, K, au, bu, cf, 1), 5, 2) / 1e9
+    except Exception as e:
+        out['probe_error'] = str(e)[:200]
+    try:
+        bt = b8.t()
+        out['torch_int_mm_tops'] = ops / _time_ms(torch, lambda: torch._int_mm(a8, bt), 5, 2) / 1e9
+    except Exception as e:
+        out['torch_int_mm_error'] = str(e)[:200]
     return out
 
 
-def sweep_report(api, syn, torch):
-    """BASELINE.json configs[4]: H=24, D=128, N in {4096..131072}; per-N kernel ms / TOPS and the blended per-step time of
-    a 50-step schedule with the FP16 fallback on the first 5 steps and on round(0.1 H) seeded heads."""
+VARIANTS = [  # name, kwargs of api.params_for
+    ('half_asym15', dict(rot_mode=2, p_mode=0)),
+    ('interleaved_asym15', dict(rot_mode=1, p_mode=0)),
+    ('full_asym15', dict(rot_mode=3, p_mode=0)),
+    ('none_asym15', dict(rot_mode=0, p_mode=0)),
+    ('naive_none_sym7', dict(rot_mode=0, p_mode=1)),
+    ('half_asym15_qkblock128', dict(rot_mode=2, p_mode=0, qk_group=128)),
+    ('half_asym15_qkblock128_vgroup', dict(rot_mode=2, p_mode=0, qk_group=128, v_scale=1)),
+    ('half_asym15_smooth', dict(rot_mode=2, p_mode=0, smooth=1)),
+]
+
+
+def quality_report(api, syn, torch, workloads, heads=(0, 1), n_tiles=2):
+    """Runs inside the cpu_baseline leg (the oracle is executed here): INT4 output against EXACT attention (oracle o_exact in
+    fp64 on the parity row sample: 2 heads x n_tiles query tiles x all keys) for every config, the headline mode beside
+    the naive symmetric-INT4 / no-rotation baseline and the f1 / f2 / f3 variants; the FP16 kernel's raw max-abs error and
+    the share of elements above 2e-3; max Psi (Eq.2) before / after rotation."""
+    from oracle import rotattn_oracle as orc
+    rep = {}
+    for w in workloads:
+        hs = [h for h in heads if h < w.H]
+        q, k, v = syn.gen_all(w, heads=hs)
+        Q, K, V = (torch.from_numpy(x).cuda() for x in (q, k, v))
+        po = orc.Params(w.B, len(hs), w.N, w.D, w.grid, w.pairs, rot_mode=orc.ROT_NONE)
+        rows_h = [syn.sample_rows(w, n_tiles=n_tiles, head=h) for h in hs]
+        exact = []
+        for i in range(len(hs)):
+            qr = orc.rope_fp64_pairs(po, q[0, i].astype(np.float64))[rows_h[i]]
+            kr = orc.rope_fp64_pairs(po, k[0, i].astype(np.float64))
+            exact.append(orc.o_exact(qr, kr, v[0, i].astype(np.float64)))
+        ex = np.concatenate(exact)
+
+        def metrics(o):
+            o = o.astype(np.float64)
+            return {'cosine': float((o * ex).sum() / (np.linalg.norm(o) * np.linalg.norm(ex))),
+                    'rel_l1': float(np.abs(o - ex).sum() / np.abs(ex).sum())}
+        entry = {}
+        for name, kw in VARIANTS:
+            p = api.params_for(w, H=len(hs), **kw)
+            cf = torch.from_numpy(api.rotattn_build_tables(p)).cuda()
+            bb = api.Buffers(p, want_fp16=(name == 'half_asym15'))
+            if kw.get('smooth'):
+                api.rotattn_smooth_stats(p, cf, None, Q, K, V, bb.ws)
+            api.rotattn_prepare_qk(p, cf, None, Q, K, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.Q16, bb.K16, bb.ws)
+            api.rotattn_quant_v(p, V, bb.V4, bb.Vs, bb.ws)
+            api.rotattn_fwd_int4(p, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.V4, bb.Vs, bb.O, bb.ws, api.WS_HAS_QK | api.WS_HAS_V)
+            torch.cuda.synchronize()
+            o = np.concatenate([bb.O[0, i].float().cpu().numpy()[rows_h[i]] for i in range(len(hs))])
+            entry[name] = metrics(o)
+            if name == 'half_asym15':
+                api.rotattn_fwd_fp16(p, bb.Q16, bb.K16, V, bb.O16, bb.ws16)
+                torch.cuda.synchronize()
+                o16 = np.concatenate([bb.O16[0, i].float().cpu().numpy()[rows_h[i]] for i in range(len(hs))]).astype(np.float64)
+                # exact attention on exactly the fp16 tensors the kernel consumed (its parity reference, DESIGN.md reading 25)
+                ex16 = np.concatenate([orc.o_exact(bb.Q16[0, i].cpu().numpy().astype(np.float64)[rows_h[i]],
+                                                   bb.K16[0, i].cpu().numpy().astype(np.float64), v[0, i].astype(np.float64))
+                                       for i in range(len(hs))])
+                err = np.abs(o16 - ex16)
+                entry['fp16_kernel'] = {'max_abs_err': float(err.max()), 'share_above_2e-3': float((err > 2e-3).mean()),
+                                        'max_abs_O': float(np.abs(ex16).max()), **metrics(o16)}
+            del bb
+        psi = {}
+        for name, mode in (('none', orc.ROT_NONE), ('interleaved', orc.ROT_INTERLEAVED), ('half', orc.ROT_HALF), ('full', orc.ROT_FULL)):
+            pm = orc.Params(1, 1, w.N, w.D, w.grid, w.pairs, rot_mode=mode)
+            psi[name] = float(orc.incoherence(orc.apply_rope_rot(pm, q[0, 0], orc.coef_table(pm))).max())
+        entry['psi_max_q_head0'] = psi
+        entry['sample'] = f'heads {hs}, {n_tiles} query tiles each (incl. the ragged last tile) x all {w.N} keys'
+        rep[w.name] = entry
+        del Q, K, V
+        torch.cuda.empty_cache()
+    rep['note'] = ('synthetic outlier inputs (stand-ins for Wan2.2 / HunyuanVideo activations); the paper reports video-level metrics '
+                   'only (Table 1); reference = oracle o_exact (fp64) on fp64-RoPE of the fp16 inputs')
+    return rep
+
+
+def sweep_report(api, syn, torch, local):
+    """BASELINE.json configs[4]: H=24, D=128, N in {4096..131072} on the cfg-5 generator; per-N kernel ms / TOPS, the blended
+    per-step time of a 50-step schedule with the FP16 fallback on the first 5 steps and on round(0.1 H) seeded heads (the two
+    head subsets launched on two streams, so that the FP16 CTAs fill the last partial wave of the INT4 launch), the same step
+    replayed as a CUDA graph, and a clocks record per point."""
     rows = []
+    s2 = torch.cuda.Stream()
     for w in syn.SWEEP:
-        p = api.params_for(w, api.ROT_HALF)
+        p = api.params_for(w, rot_mode=api.ROT_HALF)
         B, H, N, D = w.B, w.H, w.N, w.D
-        g = torch.Generator(device='cuda').manual_seed(w.seed)
-        Q, K, V = (torch.randn((B, H, N, D), device='cuda', dtype=torch.float16, generator=g) for _ in range(3))
+        q, k, v = syn.gen_all(w)
+        Q, K, V = (torch.from_numpy(x).cuda() for x in (q, k, v))
+        del q, k, v
         cf = torch.from_numpy(api.rotattn_build_tables(p)).cuda()
         bb = api.Buffers(p, want_fp16=True)
         rng = np.random.Generator(np.random.PCG64(w.seed + 2))
@@ -151,20 +281,82 @@ def sweep_report(api, syn, torch):
         sel16, sel4 = torch.from_numpy(f16_heads).cuda(), torch.from_numpy(i4_heads).cuda()
         it = 3 if N >= 65536 else 10
         ws_state = api.WS_HAS_QK | api.WS_HAS_V
+        sampler = ClockSampler(local)
+        sampler.start()
+        sampler.mark(True)
         t_prep = _time_ms(torch, lambda: api.rotattn_prepare_qk(p, cf, None, Q, K, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.Q16, bb.K16, bb.ws), it)
         t_qv = _time_ms(torch, lambda: api.rotattn_quant_v(p, V, bb.V4, bb.Vs, bb.ws), it)
         t_i4 = _time_ms(torch, lambda: api.rotattn_fwd_int4(p, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.V4, bb.Vs, bb.O, bb.ws, ws_state), it)
         t_f16 = _time_ms(torch, lambda: api.rotattn_fwd_fp16(p, bb.Q16, bb.K16, V, bb.O16, bb.ws16), it)
         t_i4s = _time_ms(torch, lambda: api.rotattn_fwd_int4(p, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.V4, bb.Vs, bb.O, bb.ws, ws_state, head_sel=sel4), it)
         t_f16s = _time_ms(torch, lambda: api.rotattn_fwd_fp16(p, bb.Q16, bb.K16, V, bb.O, bb.ws16, head_sel=sel16), it)
+
+        def mixed_step():
+            """prepare -> quant -> {INT4 heads | FP16 heads on a second stream}, joined"""
+            cur = torch.cuda.current_stream()
+            api.rotattn_prepare_qk(p, cf, None, Q, K, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.Q16, bb.K16, bb.ws)
+            s2.wait_stream(cur)
+            with torch.cuda.stream(s2):
+                api.rotattn_fwd_fp16(p, bb.Q16, bb.K16, V, bb.O, bb.ws16, head_sel=sel16, stream=s2)
+            api.rotattn_quant_v(p, V, bb.V4, bb.Vs, bb.ws)
+            api.rotattn_fwd_int4(p, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.V4, bb.Vs, bb.O, bb.ws, ws_state, head_sel=sel4)
+            cur.wait_stream(s2)
+        t_mixed = _time_ms(torch, mixed_step, it, warm=2)
+        t_graph = None
+        try:
+            gs = torch.cuda.Stream()
+            with torch.cuda.stream(gs):
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=gs):
+                    mixed_step()
+                torch.cuda.synchronize()
+                t_graph = _time_ms(torch, g.replay, it, warm=2)
+            del g
+        except Exception as e:
+            t_graph = f'capture failed: {str(e)[:120]}'
+        sampler.mark(False)
+        clocks = sampler.stop()
         ops = 4.0 * B * H * N * N * D
-        blended = (5 * (t_prep + t_f16) + 45 * (t_prep + t_qv + t_i4s + t_f16s)) / 50
+        blended_serial = (5 * (t_prep + t_f16) + 45 * (t_prep + t_qv + t_i4s + t_f16s)) / 50
+        blended = (5 * (t_prep + t_f16) + 45 * t_mixed) / 50
         rows.append({'N': N, 'prepare_qk_ms': t_prep, 'quant_v_ms': t_qv, 'fwd_int4_ms': t_i4, 'fwd_int4_tops': ops / t_i4 / 1e9,
                      'fwd_fp16_ms': t_f16, 'fwd_fp16_tflops': ops / t_f16 / 1e9, 'int4_heads': len(i4_heads), 'fp16_heads': len(f16_heads),
-                     'fwd_int4_subset_ms': t_i4s, 'fwd_fp16_subset_ms': t_f16s, 'blended_step_ms': blended, 'all_fp16_step_ms': t_prep + t_f16})
+                     'fwd_int4_subset_ms': t_i4s, 'fwd_fp16_subset_ms': t_f16s, 'mixed_step_two_streams_ms': t_mixed,
+                     'mixed_step_cuda_graph_ms': t_graph, 'blended_step_ms': blended, 'blended_step_serial_launches_ms': blended_serial,
+                     'all_fp16_step_ms': t_prep + t_f16, 'prologue_pct_of_int4_attention': 100.0 * (t_prep + t_qv) / t_i4,
+                     'clocks': {k: clocks.get(k) for k in ('sm_mhz', 'sm_mhz_min', 'reasons', 'samples')}})
         del Q, K, V, bb
         torch.cuda.empty_cache()
     return rows
+
+
+def variants_report(api, torch, w, Q, K, V, ops, iters):
+    """ms / TOPS / fraction of the 8-bit roofline of every built variant of the attention kernel on the bench workload,
+    side by side with the per-token headline (p_norm = RUNNING is the serialised kernel)."""
+    out = {}
+    pk = _peaks()
+    cases = [('per_token_channel (headline)', {}), ('qk_block128', dict(qk_group=128)), ('v_group_scalar', dict(v_scale=1)),
+             ('qk_block128_v_group', dict(qk_group=128, v_scale=1)), ('sym7', dict(p_mode=1)), ('smooth', dict(smooth=1)),
+             ('rot_full (prologue only differs)', dict(rot_mode=3)), ('p_norm_running', dict(p_norm=1))]
+    for name, kw in cases:
+        kw = dict(kw)
+        rot_mode = kw.pop('rot_mode', api.ROT_HALF)
+        p = api.params_for(w, rot_mode=rot_mode, **kw)
+        cf = torch.from_numpy(api.rotattn_build_tables(p)).cuda()
+        bb = api.Buffers(p)
+        t_stats = None
+        if kw.get('smooth'):
+            t_stats = _time_ms(torch, lambda: api.rotattn_smooth_stats(p, cf, None, Q, K, V, bb.ws), iters)
+        t_prep = _time_ms(torch, lambda: api.rotattn_prepare_qk(p, cf, None, Q, K, bb.Q4, bb.Qs, bb.K4, bb.Ks, None, None, bb.ws), iters)
+        t_qv = _time_ms(torch, lambda: api.rotattn_quant_v(p, V, bb.V4, bb.Vs, bb.ws), iters)
+        t = _time_ms(torch, lambda: api.rotattn_fwd_int4(p, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.V4, bb.Vs, bb.O, bb.ws, api.WS_HAS_QK | api.WS_HAS_V), iters, warm=2)
+        tops = ops / t / 1e9
+        out[name] = {'fwd_int4_ms': t, 'tops': tops, 'frac_of_2x_bf16_measured': tops / (2.0 * pk['bf16']), 'prepare_qk_ms': t_prep,
+                     'quant_v_ms': t_qv}
+        if t_stats is not None:
+            out[name]['smooth_stats_ms'] = t_stats
+        del bb
+    return out
 
 
 def run_reference(args):
@@ -184,7 +376,7 @@ def run_reference(args):
     out = {'impl': 'reference', 'metric': METRIC, 'value': val, 'unit': 'TOPS', 'n_gpus': args.gpus, 'steps': len(ts),
            'warmup': min(warm, 1), 'ms_per_step': dt * 1e3, 'higher_is_better': True, 'scaling': 'weak', 'vs_baseline': None,
            'dtype': 'f64', 'data': 'synthetic', 'config': {'workload': WORKLOAD, 'note': 'bounded sample per step: ' + sample},
-           'cpu_baseline': {'value': val, 'unit': 'TOPS', 'cores': os.cpu_count(), 'kind': 'oracle', 'sample': sample},
+           'cpu_baseline': {'value': val, 'unit': 'TOPS', 'cores': os.cpu_count(), 'kind': 'oracle', 'sample': sample, 'cpu_model': _cpu_model()},
            'e2e': {'value': val, 'unit': 'TOPS', 'h2d_bytes_per_step': 0, 'd2h_bytes_per_step': 0}, 'gpu_launches': 0}
     print(json.dumps(out))
 
@@ -195,17 +387,24 @@ def main():
     ap.add_argument('--steps', type=int, default=10)
     ap.add_argument('--warmup', type=int, default=3)
     ap.add_argument('--impl', default='ours')
+    ap.add_argument('--rows', type=int, default=256, help='(--impl oracle-sample) query rows of the one-thread oracle sample')
     ap.add_argument('--no-cpu-baseline', action='store_true')
-    ap.add_argument('--no-extras', action='store_true', help='skip the quality report and the N sweep (configs[4])')
+    ap.add_argument('--no-extras', action='store_true', help='skip the quality report, the variants table and the N sweep (configs[4])')
+    ap.add_argument('--head-shard', action='store_true', help='N > 1: split the heads of one workload over the ranks (strong scaling)')
     args = ap.parse_args()
     if args.impl == 'reference':
         return run_reference(args)
+    if args.impl == 'oracle-sample':     # helper leg of cpu_baseline (one BLAS thread)
+        dt, cops, nrows = cpu_oracle_sample(args.rows)
+        print(json.dumps({'value': cops / dt / 1e12, 'unit': 'TOPS', 'threads': 1, 'rows': nrows, 'seconds': dt}))
+        return
 
     import torch
     import torch.distributed as dist
     import __graft_entry__ as entry
     entry.build()
     from paper_2607_02584_b200 import api
+    from paper_2607_02584_b200 import dist as rdist
     from synth import video_qkv as syn
 
     world = int(os.environ.get('WORLD_SIZE', '1'))
@@ -217,10 +416,21 @@ def main():
     W = max(3, args.warmup)
     K = args.steps
     w = syn.ALL[WORKLOAD]
-    p = api.params_for(w, api.ROT_HALF)
+    p = api.params_for(w, rot_mode=api.ROT_HALF)
     B, H, N, D = w.B, w.H, w.N, w.D
-    ops = 4.0 * B * H * N * N * D
+    ops_full = 4.0 * B * H * N * N * D
+    # --head-shard: this rank's contiguous head range (no data-path collective)
+    head_sel = None
+    my_units = B * H
+    if args.head_shard and world > 1:
+        mine = rdist.shard_heads(B * H, world, rank)
+        head_sel = torch.from_numpy(mine).cuda()
+        my_units = len(mine)
+    ops = ops_full * my_units / (B * H)
 
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
     # synthetic inputs of the BASELINE.json recipe (every replica runs the same seeded tensors)
     q, k, v = syn.gen_all(w)
     hq, hk, hv = (torch.from_numpy(x).pin_memory() for x in (q, k, v))
@@ -229,34 +439,26 @@ def main():
     b = api.Buffers(p, want_fp16=True)
     hO = torch.empty((B, H, N, D), dtype=torch.float16).pin_memory()
     stream = torch.cuda.current_stream()
+    ws_state = api.WS_HAS_QK | api.WS_HAS_V
 
     def step():
         api.rotattn_prepare_qk(p, coef, None, Q, Kt, b.Q4, b.Qs, b.K4, b.Ks, None, None, b.ws)
         api.rotattn_quant_v(p, V, b.V4, b.Vs, b.ws)
-        api.rotattn_fwd_int4(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, b.O, b.ws, api.WS_HAS_QK | api.WS_HAS_V)
+        api.rotattn_fwd_int4(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, b.O, b.ws, ws_state, head_sel=head_sel)
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    def max_over_ranks(ms):
-        if world > 1:
-            t = torch.tensor([ms], device='cuda')
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            return float(t.item())
-        return ms
-
     for _ in range(W):
         step()
     barrier()
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
     # ---- timed region: K steps, per-kernel CUDA events on the launching stream
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(K)]
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
+    sampler.mark(True)
     e0.record(stream)
     for i in range(K):
         ev[i][0].record(stream)
@@ -264,16 +466,31 @@ def main():
         ev[i][1].record(stream)
         api.rotattn_quant_v(p, V, b.V4, b.Vs, b.ws)
         ev[i][2].record(stream)
-        api.rotattn_fwd_int4(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, b.O, b.ws, api.WS_HAS_QK | api.WS_HAS_V)
+        api.rotattn_fwd_int4(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, b.O, b.ws, ws_state, head_sel=head_sel)
         ev[i][3].record(stream)
     e1.record(stream)
     barrier()
-    total_ms = max_over_ranks(e0.elapsed_time(e1))
-    clocks = sampler.stop() if rank == 0 else None
+    sampler.mark(False)
+    total_ms = rdist.max_over_ranks(e0.elapsed_time(e1), device='cuda')
     t_prep = float(np.mean([ev[i][0].elapsed_time(ev[i][1]) for i in range(K)]))
     t_qv = float(np.mean([ev[i][1].elapsed_time(ev[i][2]) for i in range(K)]))
     t_int4 = float(np.mean([ev[i][2].elapsed_time(ev[i][3]) for i in range(K)]))
     ms_step = total_ms / K
+    value_tops = rdist.aggregate_throughput(ops * K, e0.elapsed_time(e1), device='cuda') / 1e12
+
+    # ---- the same step as ONE CUDA graph (prepare -> quant -> attention captured once, replayed)
+    graph_ms = None
+    try:
+        gs = torch.cuda.Stream()
+        with torch.cuda.stream(gs):
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=gs):
+                step()
+            torch.cuda.synchronize()
+            graph_ms = _time_ms(torch, g.replay, max(3, K), warm=2)
+        del g
+    except Exception as e:
+        graph_ms = f'capture failed: {str(e)[:120]}'
 
     # ---- FP16 fallback kernel (speed-up denominator), same shapes
     api.rotattn_prepare_qk(p, coef, None, Q, Kt, b.Q4, b.Qs, b.K4, b.Ks, b.Q16, b.K16, b.ws)
@@ -296,26 +513,25 @@ def main():
     ev_in = [torch.cuda.Event() for _ in range(2)]
     ev_c = [torch.cuda.Event() for _ in range(2)]
     ev_out = [torch.cuda.Event() for _ in range(2)]
-    ws_state = api.WS_HAS_QK | api.WS_HAS_V
 
     def e2e_run(n):
         for i in range(n):
-            k = i & 1
+            kk = i & 1
             with torch.cuda.stream(s_in):
-                s_in.wait_event(ev_c[k])                      # the step that last read these input buffers is done
-                Qd[k].copy_(hq, non_blocking=True); Kd[k].copy_(hk, non_blocking=True); Vd[k].copy_(hv, non_blocking=True)
-                ev_in[k].record(s_in)
+                s_in.wait_event(ev_c[kk])                      # the step that last read these input buffers is done
+                Qd[kk].copy_(hq, non_blocking=True); Kd[kk].copy_(hk, non_blocking=True); Vd[kk].copy_(hv, non_blocking=True)
+                ev_in[kk].record(s_in)
             with torch.cuda.stream(s_c):
-                s_c.wait_event(ev_in[k])
-                s_c.wait_event(ev_out[k])                     # the result buffer has been copied out
-                api.rotattn_prepare_qk(p, coef, None, Qd[k], Kd[k], b.Q4, b.Qs, b.K4, b.Ks, None, None, b.ws, stream=s_c)
-                api.rotattn_quant_v(p, Vd[k], b.V4, b.Vs, b.ws, stream=s_c)
-                api.rotattn_fwd_int4(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, Od[k], b.ws, ws_state, stream=s_c)
-                ev_c[k].record(s_c)
+                s_c.wait_event(ev_in[kk])
+                s_c.wait_event(ev_out[kk])                     # the result buffer has been copied out
+                api.rotattn_prepare_qk(p, coef, None, Qd[kk], Kd[kk], b.Q4, b.Qs, b.K4, b.Ks, None, None, b.ws, stream=s_c)
+                api.rotattn_quant_v(p, Vd[kk], b.V4, b.Vs, b.ws, stream=s_c)
+                api.rotattn_fwd_int4(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, Od[kk], b.ws, ws_state, head_sel=head_sel, stream=s_c)
+                ev_c[kk].record(s_c)
             with torch.cuda.stream(s_out):
-                s_out.wait_event(ev_c[k])
-                hO.copy_(Od[k], non_blocking=True)
-                ev_out[k].record(s_out)
+                s_out.wait_event(ev_c[kk])
+                hO.copy_(Od[kk], non_blocking=True)
+                ev_out[kk].record(s_out)
     e2e_run(2)
     barrier()
     g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -325,57 +541,79 @@ def main():
     s_out.wait_stream(s_c); s_out.wait_stream(s_in)
     g1.record(s_out)
     barrier()
-    e2e_ms = max_over_ranks(g0.elapsed_time(g1)) / ne
+    e2e_local = g0.elapsed_time(g1)
+    e2e_ms = rdist.max_over_ranks(e2e_local, device='cuda') / ne
+    e2e_tops = rdist.aggregate_throughput(ops * ne, e2e_local, device='cuda') / 1e12
     h2d = 3 * B * H * N * D * 2
     d2h = B * H * N * D * 2
+    clocks = sampler.stop() if rank == 0 else None
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
     pk = _peaks()
-    quality = sweep = None
-    if not args.no_extras and world == 1:
-        quality = quality_report(api, syn, torch, w, Q, Kt, V, b, coef)
-        del hq, hk, hv, hO
-        sweep = sweep_report(api, syn, torch)
+    extras = not args.no_extras and world == 1
+    variants = sweep = peaks8 = None
+    if extras:
+        peaks8 = measured_8bit_peaks(api, torch)
+        variants = variants_report(api, torch, w, Q, Kt, V, ops_full, max(3, min(K, 10)))
     int8_peak = 2.0 * pk['bf16']      # dense int8 = 2x bf16 nominal ratio (4.5 / 2.25 PFLOP/s) applied to the measured bf16 peak
     achieved = ops / (t_int4 * 1e-3) / 1e12
-    traffic = None
+    traffic = traffic_src = None
     tpath = os.path.join(ROOT, 'profiles', 'fwd_int4_traffic.csv')     # dram__bytes_read+write of one ncu --set full capture
     if os.path.exists(tpath):
-        last = open(tpath).read().strip().splitlines()[-1].split(',')
+        lines = open(tpath).read().strip().splitlines()
+        last = lines[-1].split(',')
         traffic = int(last[-2]) if last[-2].isdigit() else None
+        traffic_src = 'profiles/fwd_int4_traffic.csv (' + last[0] + '); an ncu capture of an earlier run of this command, not of this run'
     out = {
-        'metric': METRIC, 'value': world * ops / (ms_step * 1e-3) / 1e12, 'unit': 'TOPS', 'n_gpus': world, 'steps': K, 'warmup': W,
-        'ms_per_step': ms_step, 'higher_is_better': True, 'scaling': 'weak', 'vs_baseline': None, 'dtype': 'int8 codes (INT4 values) / int32 accumulate / fp32 softmax',
-        'data': 'synthetic',
+        'metric': METRIC, 'value': value_tops, 'unit': 'TOPS', 'n_gpus': world, 'steps': K, 'warmup': W,
+        'ms_per_step': ms_step, 'higher_is_better': True, 'scaling': 'strong' if args.head_shard and world > 1 else 'weak',
+        'vs_baseline': None, 'dtype': DTYPE, 'data': 'synthetic',
         'config': {'workload': WORKLOAD, 'B': B, 'H': H, 'N': N, 'D': D, 'grid': list(w.grid), 'rot_mode': 'HALF', 'p_mode': 'ASYM15',
-                   'p_norm': 'ROWBLOCK', 'l2': 'inputs larger than L2 (Q,K,V fp16 = 302 MB per step; no flush)',
-                   'parallelism': f'replicas x{world} (independent (b,h) units, no collective)'},
+                   'p_norm': 'ROWBLOCK', 'qk_group': 1, 'v_scale': 'per (128-token group, channel)',
+                   'l2': 'inputs larger than L2 (Q,K,V fp16 = 302 MB per step; no flush)',
+                   'parallelism': (f'heads sharded over {world} ranks (no collective)' if args.head_shard and world > 1
+                                   else f'replicas x{world} (independent (b,h) units, no collective)')},
         'kernels_ms': {'prepare_qk': t_prep, 'quant_v': t_qv, 'fwd_int4': t_int4, 'fwd_fp16': t_fp16},
+        'step_as_cuda_graph_ms': graph_ms,
         'int4_kernel_tops': achieved, 'fp16_kernel_tflops': ops / (t_fp16 * 1e-3) / 1e12,
+        'fp16_kernel_frac_of_measured_bf16': ops / (t_fp16 * 1e-3) / 1e12 / pk['bf16'],
         'speedup_int4_vs_own_fp16_kernel': t_fp16 / t_int4,
-        'prologue_gbs': {'prepare_qk': (2 * (2 * D + D // 2 + 4 + 128) * B * H * N) / (t_prep * 1e-3) / 1e9,
+        'prologue_pct_of_int4_attention': 100.0 * (t_prep + t_qv) / t_int4,
+        'prologue_gbs': {'prepare_qk': (2 * (2 * D + D // 2 + 4 + 128 + 4) * B * H * N) / (t_prep * 1e-3) / 1e9,
                          'quant_v': ((2 * D + D // 2 + D) * B * H * N + 4 * D * B * H * ((N + 127) // 128)) / (t_qv * 1e-3) / 1e9,
                          'peak': pk['hbm']},
         'roofline': {'kernel': 'fwd_int4_kernel', 'bound': 'tensor', 'achieved': achieved, 'peak': int8_peak, 'unit': 'TOPS',
-                     'frac': achieved / int8_peak, 'traffic': traffic,
-                     'peak_source': f"2 x bf16_tflops ({pk['bf16']}) of {pk['src']} (dense int8:bf16 nominal ratio 2; of measured)"},
-        'e2e': {'value': world * ops / (e2e_ms * 1e-3) / 1e12, 'unit': 'TOPS', 'ms_per_step': e2e_ms, 'how': 'C-ABI calls on pinned-host inputs; H2D / compute / D2H streams over double-buffered device tensors, every step copies all inputs in and O out',
+                     'frac': achieved / int8_peak, 'traffic': traffic, 'traffic_source': traffic_src,
+                     'peak_source': f"2 x bf16_tflops ({pk['bf16']}) of {pk['src']} (dense 8-bit : bf16 nominal ratio 2; of measured)",
+                     'measured_8bit_gemm_peaks_this_run': peaks8},
+        'e2e': {'value': e2e_tops, 'unit': 'TOPS', 'ms_per_step': e2e_ms, 'how': 'C-ABI calls on pinned-host inputs; H2D / compute / D2H streams over double-buffered device tensors, every step copies all inputs in and O out',
                 'h2d_bytes_per_step': h2d, 'd2h_bytes_per_step': d2h},
         'gpu_launches': 3 * K,
         'clocks': clocks,
         'paper_context': 'paper: up to 2.2x INT4 vs its FP16 kernel on A10, 1.68x end to end (PAPER.md:L267) - other hardware',
     }
-    if quality is not None:
-        out['quality_vs_own_fp16_kernel'] = quality
-    if sweep is not None:
-        out['sweep_mixed_precision'] = sweep
+    if variants is not None:
+        out['variants'] = variants
     if not args.no_cpu_baseline and world == 1:
-        dt, cops, nrows = cpu_oracle_sample(16384)
-        out['cpu_baseline'] = {'value': cops / dt / 1e12, 'unit': 'TOPS', 'cores': os.cpu_count(), 'kind': 'oracle', 'seconds': dt,
-                               'sample': f'{WORKLOAD}: 1 head, full prologue on N={N} tokens + O-quant for {nrows} query rows x all keys'}
+        cb = cpu_baseline_block(16384, B * H * N)
+        if extras:
+            # quality against exact attention (oracle o_exact) belongs to this leg: it is where the oracle runs
+            try:
+                cb['quality_vs_o_exact'] = quality_report(api, syn, torch, [syn.TINY, syn.WAN_1_3B, syn.WAN_14B, syn.HUNYUAN,
+                                                                                syn.SWEEP[0], syn.SWEEP[1], syn.SWEEP[3]])
+            except Exception as e:
+                cb['quality_vs_o_exact'] = {'error': str(e)[:300]}
+        out['cpu_baseline'] = cb
+    if extras:
+        del hq, hk, hv, hO, Q, Kt, V, b, Qd, Kd, Vd, Od
+        torch.cuda.empty_cache()
+        try:
+            out['sweep_mixed_precision'] = sweep_report(api, syn, torch, local)
+        except Exception as e:
+            out['sweep_mixed_precision'] = {'error': str(e)[:300]}
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()

@@ -254,6 +254,29 @@ def rope_fp64(p: Params, x, rot_mode=ROT_NONE, rot=None):
     return y
 
 
+def rope_fp64_pairs(p: Params, x, rot_mode=ROT_NONE, rot=None):
+    """Same map as rope_fp64, evaluated pair by pair (y0 = x0 c - x1 s, y1 = x0 s + x1 c, L60) on whole arrays instead of one
+    dense D x D matrix per token: used where N is too large for the dense form (quality references at full size).
+    Pinned against rope_fp64 in tests/test_oracle_pins.py."""
+    x = np.asarray(x, dtype=F64)
+    N, D = x.shape
+    t, h, w, is_rope = token_positions(p.N, p.grid)
+    pos = [t, h, w]
+    y = np.empty((N, D), dtype=F64)
+    gp = 0
+    for a in range(3):
+        P = p.pairs[a]
+        th = np.where(is_rope, pos[a], 0).astype(F64)[:, None] * rope_freqs(P, p.rope_base)[None, :]     # [N, P]
+        c, sn = np.cos(th), np.sin(th)
+        x0, x1 = x[:, 2 * gp:2 * (gp + P):2], x[:, 2 * gp + 1:2 * (gp + P):2]
+        y[:, 2 * gp:2 * (gp + P):2] = x0 * c - x1 * sn
+        y[:, 2 * gp + 1:2 * (gp + P):2] = x0 * sn + x1 * c
+        gp += P
+    if rot_mode != ROT_NONE:
+        y = y @ dense_rotation(p, rot_mode, rot)
+    return y
+
+
 def dense_rotation(p: Params, rot_mode, rot=None):
     """The D x D orthogonal matrix (Pi R) of Eq.3 (INTERLEAVED) or Eq.8 (HALF) as a dense matrix."""
     D = p.D

@@ -276,3 +276,47 @@ def test_batch_of_two_and_d64_many_tiles():
             ph.check_o(res['O'][bi, h].float().cpu().numpy(),
                        orc.o_quant(po, pq['q_codes'], pq['q_scale'], pq['k_codes'], pq['k_scale'], vc, vs))
     ph.check_tile(res, po, 1, 1, 8)
+
+
+def test_cuda_graph_capture_of_the_step():
+    """prepare_qk -> quant_v -> fwd_int4 (+ the FP16 head subset on a forked stream) captured once as a
+    CUDA graph; the replay reproduces the eager result bit for bit (the library enqueues only, never synchronises)."""
+    api = ph.api()
+    w = syn.small_variant(syn.SWEEP[0], (4, 16, 16), H=4)          # N = 1024
+    q, k, v = syn.gen_all(w)
+    p = api.params_for(w, rot_mode=orc.ROT_HALF)
+    coef = torch.from_numpy(api.rotattn_build_tables(p)).cuda()
+    Q, K, V = (torch.from_numpy(x).cuda() for x in (q, k, v))
+    b = api.Buffers(p, want_fp16=True)
+    sel4 = torch.tensor([0, 2, 3], dtype=torch.int32, device='cuda')
+    sel16 = torch.tensor([1], dtype=torch.int32, device='cuda')
+    s2 = torch.cuda.Stream()
+    O = torch.zeros_like(b.O)
+
+    def step(out):
+        cur = torch.cuda.current_stream()
+        api.rotattn_prepare_qk(p, coef, None, Q, K, b.Q4, b.Qs, b.K4, b.Ks, b.Q16, b.K16, b.ws)
+        s2.wait_stream(cur)
+        with torch.cuda.stream(s2):
+            api.rotattn_fwd_fp16(p, b.Q16, b.K16, V, out, b.ws16, head_sel=sel16, stream=s2)
+        api.rotattn_quant_v(p, V, b.V4, b.Vs, b.ws)
+        api.rotattn_fwd_int4(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, out, b.ws, api.WS_HAS_QK | api.WS_HAS_V, head_sel=sel4)
+        cur.wait_stream(s2)
+    step(O)                                        # eager (also warms up the per-kernel attribute setup)
+    torch.cuda.synchronize()
+    want = O.clone()
+    O2 = torch.zeros_like(O)
+    gs = torch.cuda.Stream()
+    with torch.cuda.stream(gs):
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=gs):
+            step(O2)
+        torch.cuda.synchronize()
+        assert torch.all(O2 == 0)                  # capture does not execute
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(O2, want)
+        O2.zero_()
+        g.replay(); g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(O2, want)

@@ -111,6 +111,14 @@ def test_rope_textbook_properties():
     assert np.allclose(y[:, 0::2], z.real, atol=1e-10) and np.allclose(y[:, 1::2], z.imag, atol=1e-10)
 
 
+def test_rope_pairwise_form_equals_dense_form():
+    p = _params(N=N0 + 4)
+    rng = np.random.default_rng(36)
+    x = rng.standard_normal((p.N, p.D))
+    for mode in (orc.ROT_NONE, orc.ROT_HALF, orc.ROT_FULL):
+        assert np.abs(orc.rope_fp64_pairs(p, x, mode) - orc.rope_fp64(p, x, mode)).max() <= 1e-12
+
+
 def test_rope_relative_position_property():
     """Shifting every position of one axis by a constant leaves Q_r K_r^T unchanged."""
     p = _params()
