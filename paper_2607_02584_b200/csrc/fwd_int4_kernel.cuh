@@ -197,7 +197,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const int m = i, j = i - 2;                                      // K runs two blocks ahead of V
         if (m < nblk) {
           const int s = m % K_STAGES;
-          mbar_wait(&s_done[s], ((m / K_STAGES) & 1) ^ 1);               // S(m-4) has consumed this K stage
+          mbar_wait_hint(&s_done[s], ((m / K_STAGES) & 1) ^ 1);               // S(m-4) has consumed this K stage
           if (elect_one()) {
             mbar_arrive_expect_tx(&k_full[s], L::K_BYTES);
             tma_load_3d(sK + s * L::K_BYTES, &tmK, &k_full[s], 0, m * kTile, bh);
@@ -206,7 +206,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         }
         if (j >= 0) {
           const int s = j % V_STAGES;
-          if (j >= V_STAGES) mbar_wait(&pv_done[(j - V_STAGES) % P_SLOTS], ((j - V_STAGES) / P_SLOTS) & 1);   // P~V(j-3) has consumed this V stage
+          if (j >= V_STAGES) mbar_wait_hint(&pv_done[(j - V_STAGES) % P_SLOTS], ((j - V_STAGES) / P_SLOTS) & 1);   // P~V(j-3) has consumed this V stage
           if (elect_one()) {
             mbar_arrive_expect_tx(&v_full[s], L::V_BYTES);
             tma_load_3d(sV + s * L::V_BYTES, &tmV, &v_full[s], j * kTile, 0, bh);
@@ -219,11 +219,11 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       constexpr uint32_t idesc_s = umma_idesc(1, 0, 0, 128, 128);        // f32 <- e4m3 x e4m3 (integer codes * 2^-9)
       constexpr int KSTEPS_S = D / 32;                                   // D=64 rows are zero-padded to 128 B
       const uint64_t qd = umma_desc_k128(smem_u32(sQ));
-      mbar_wait(q_full, 0);
+      mbar_wait_hint(q_full, 0);
       for (int m = 0; m < nblk; ++m) {
         const int st = m % K_STAGES, b = m & 1;
-        mbar_wait(&k_full[st], (m / K_STAGES) & 1);
-        if (m >= 2) mbar_wait(&s_empty[b], ((m >> 1) - 1) & 1);          // softmax has read S(m-2) out of this buffer
+        mbar_wait_hint(&k_full[st], (m / K_STAGES) & 1);
+        if (m >= 2) mbar_wait_hint(&s_empty[b], ((m >> 1) - 1) & 1);          // softmax has read S(m-2) out of this buffer
         tc_fence_after();
         if (elect_one()) {
           const uint64_t kd = umma_desc_k128(smem_u32(sK + st * L::K_BYTES));
@@ -239,12 +239,12 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       constexpr uint32_t idesc_pv = umma_idesc(1, 0, 0, 128, D / 2);
       for (int j = 0; j < nblk; ++j) {
         const int slot = j % P_SLOTS, vst = j % V_STAGES;
-        mbar_wait(&v_full[vst], (j / V_STAGES) & 1);
-        mbar_wait(&p_full[slot], (j / P_SLOTS) & 1);
+        mbar_wait_hint(&v_full[vst], (j / V_STAGES) & 1);
+        mbar_wait_hint(&p_full[slot], (j / P_SLOTS) & 1);
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
           const int buf = 2 * (j & 1) + h;
-          mbar_wait(&pvh_empty[buf], ((j >> 1) & 1) ^ 1);                // drain has read half (j-2, h) out of this buffer
+          mbar_wait_hint(&pvh_empty[buf], ((j >> 1) & 1) ^ 1);                // drain has read half (j-2, h) out of this buffer
           tc_fence_after();
           if (elect_one()) {
             // V^T tile: channel half h starts D/2 rows (= D/2 * 128 B, whole 1024-byte swizzle atoms) into the tile
@@ -266,13 +266,12 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       if (QKG == 1 || VSC == 0) {
         for (int j = 0; j < nblk; ++j) {
           const int s = j % KS_RING;
-          float kv[4], kc[4], vv[D / 32];
+          float kv[4], vv[D / 32];
           if (QKG == 1) {
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
               const int kj = j * kTile + i * 32 + lane;
               kv[i] = (kj < a.N) ? ksrc[kj] * a.scale_log2 : 0.f;
-              if (SM) kc[i] = (kj < a.N) ? a.KcP[(size_t)bh * a.npad + kj] : 0.f;
             }
           }
           if (VSC == 0) {
@@ -280,16 +279,20 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             for (int i = 0; i < D / 32; ++i) vv[i] = vsrc[(size_t)j * D + i * 32 + lane];
           }
           if (QKG == 1) {
-            mbar_wait(&ks_empty[s], ((j / KS_RING) & 1) ^ 1);
+            mbar_wait_hint(&ks_empty[s], ((j / KS_RING) & 1) ^ 1);
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-              sKs[s * 128 + i * 32 + lane] = kv[i];
-              if (SM) sKc[s * 128 + i * 32 + lane] = kc[i];
+            for (int i = 0; i < 4; ++i) sKs[s * 128 + i * 32 + lane] = kv[i];
+            if (SM) {                                    // per-key correction of the smoothing path (this warp has 24 registers:
+#pragma unroll                                          //  one value in flight at a time)
+              for (int i = 0; i < 4; ++i) {
+                const int kj = j * kTile + i * 32 + lane;
+                sKc[s * 128 + i * 32 + lane] = (kj < a.N) ? a.KcP[(size_t)bh * a.npad + kj] : 0.f;
+              }
             }
             mbar_arrive(&ks_full[s]);
           }
           if (VSC == 0) {
-            mbar_wait(&vs_empty[s], ((j / VS_RING) & 1) ^ 1);
+            mbar_wait_hint(&vs_empty[s], ((j / VS_RING) & 1) ^ 1);
 #pragma unroll
             for (int i = 0; i < D / 32; ++i) sVs[s * D + i * 32 + lane] = vv[i];
             mbar_arrive(&vs_full[s]);
@@ -318,7 +321,6 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       const int n = j >> 1;
       const int ring = j % KS_RING, slot = j % P_SLOTS, abslot = j % AB_RING;
       const float2* ks2 = reinterpret_cast<const float2*>(sKs + ring * 128 + cb);
-      const float2* kc2 = reinterpret_cast<const float2*>(sKc + ring * 128 + cb);
       const int nvalid = min(kTile, a.N - j * kTile) - cb;   // valid keys of this half; < 64 only on the ragged last block
       const bool ragged = nvalid < 64;
       float qs = fq;
@@ -344,7 +346,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             for (int i = 0; i < 16; ++i)
               a.S_dump[(size_t)r * a.npad + j * kTile + cb + c * 16 + i] = (int32_t)(__uint_as_float(cur[i]) * kAccScale);
           }
-          chunk_scale_max<QKG == 1, SM != 0, decltype(masked)::value>(cur, ks2 + c * 8, kc2 + c * 8, qs2, nvalid - c * 16, tt, mx0, mx1);
+          chunk_scale_max<QKG == 1, SM != 0, decltype(masked)::value>(cur, ks2 + c * 8, ks2 + c * 8 + (L::OFF_KC - L::OFF_KS) / 8, qs2, nvalid - c * 16, tt, mx0, mx1);
           if (QKG == 1) tmem_st16(s_addr + c * 16, tt);
         }
       };

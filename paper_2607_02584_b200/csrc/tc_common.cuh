@@ -68,6 +68,26 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   }
 }
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) { mbar_wait(smem_u32(bar), parity); }
+// Same wait with a suspend-time hint: the thread stays suspended in hardware until the phase completes (or the hint
+// expires) instead of returning to the retry loop - for the single-thread service roles, whose retry loops would
+// otherwise take issue slots (at the highest arbitration priority) from the softmax warps of their sub-partition.
+__device__ __forceinline__ void mbar_wait_hint(uint64_t* bar, uint32_t parity) {
+  const uint32_t addr = smem_u32(bar);
+  uint32_t spins = 0;
+#pragma unroll 1
+  for (;;) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(addr), "r"(parity), "r"(0x989680u)
+        : "memory");
+    if (ok) return;
+    if (++spins > (1u << 16)) __trap();
+  }
+}
 
 // packed fp32x2 arithmetic (sm_100: FMUL2 / FFMA2 / FADD2 issue one instruction for two lanes) and 3-input max
 __device__ __forceinline__ uint64_t pack2(float a, float b) { uint64_t r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
