@@ -286,7 +286,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 #pragma unroll                                          //  one value in flight at a time)
               for (int i = 0; i < 4; ++i) {
                 const int kj = j * kTile + i * 32 + lane;
-                sKc[s * 128 + i * 32 + lane] = (kj < a.N) ? a.KcP[(size_t)bh * a.npad + kj] : 0.f;
+                sKc[s * 128 + i * 32 + lane] = (kj < a.N) ? a.KcP[(size_t)bh * a.npad + kj] : -INFINITY;   // keys >= N: masked by the bias
               }
             }
             mbar_arrive(&ks_full[s]);
@@ -350,7 +350,8 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           if (QKG == 1) tmem_st16(s_addr + c * 16, tt);
         }
       };
-      if (ragged) pass1(std::true_type{}); else pass1(std::false_type{});
+      // smoothing: the additive per-key term is -inf for keys >= N, so the ragged block needs no separate code
+      if (ragged && !SM) pass1(std::true_type{}); else pass1(std::false_type{});
       float tmax = fmaxf(mx0, mx1);
       float* mxbuf = sMx + ((g * 2 + (n & 1)) * 2) * 128;
       mxbuf[h * 128 + r] = tmax;
