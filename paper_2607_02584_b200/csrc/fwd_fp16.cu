@@ -347,7 +347,17 @@ template <int D>
 static int launch_fp16(const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv, const FwdFp16Args& a, dim3 grid,
                        cudaStream_t cs) {
   constexpr int smem = SmemFp16<D>::TOTAL;
-  ROTATTN_CUDA_TRY(cudaFuncSetAttribute(fwd_fp16_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  static int checked = 0;       // once: ptxas must have allocated exactly the register pool setmaxnreg redistributes
+  if (!checked) {
+    cudaFuncAttributes fa;
+    ROTATTN_CUDA_TRY(cudaFuncGetAttributes(&fa, fwd_fp16_kernel<D>));
+    if (fa.numRegs != 128) {
+      set_error_text("fwd_fp16_kernel: unexpected register allocation (setmaxnreg pool assumes 128 registers per thread)");
+      return ROTATTN_ERR_UNSUPPORTED;
+    }
+    ROTATTN_CUDA_TRY(cudaFuncSetAttribute(fwd_fp16_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    checked = 1;
+  }
   fwd_fp16_kernel<D><<<grid, kFp16Threads, smem, cs>>>(tq, tk, tv, a);
   ROTATTN_CUDA_TRY(cudaGetLastError());
   return ROTATTN_OK;

@@ -319,6 +319,12 @@ static int launch_sync_variant(const rotattn_params& p, const CUtensorMap& tq, c
   constexpr int smem = SmemInt4Sync<D>::TOTAL;
 #define ROTATTN_LAUNCH(PM, PN)                                                                                      \
   do {                                                                                                              \
+    cudaFuncAttributes fa;                                                                                          \
+    ROTATTN_CUDA_TRY(cudaFuncGetAttributes(&fa, fwd_int4_sync_kernel<D, PM, PN, DEBUG>));                           \
+    if (fa.numRegs != 96) {       /* the setmaxnreg redistribution assumes a pool of 640 x 96 registers */          \
+      set_error_text("fwd_int4_sync_kernel: unexpected register allocation (setmaxnreg pool assumes 96 per thread)"); \
+      return ROTATTN_ERR_UNSUPPORTED;                                                                               \
+    }                                                                                                               \
     ROTATTN_CUDA_TRY(cudaFuncSetAttribute(fwd_int4_sync_kernel<D, PM, PN, DEBUG>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); \
     fwd_int4_sync_kernel<D, PM, PN, DEBUG><<<grid, kInt4Threads, smem, cs>>>(tq, tk, tv, a);                        \
   } while (0)
