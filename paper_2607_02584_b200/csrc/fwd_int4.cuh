@@ -6,7 +6,7 @@
 namespace rotattn {
 
 constexpr int kInt4Threads = 640;      // fwd_int4_sync_kernel
-constexpr int kFwdThreads = 896;       // fwd_int4_kernel
+constexpr int kFwdThreads = 512;       // fwd_int4_kernel
 // The widened operands are E4M3 bytes that encode code * 2^-9 (see prologue.cu: code_byte), so both tensor products
 // arrive in tensor memory as fp32 values  integer_accumulator * 2^-18  (exact: |acc| <= 13440 < 2^24;
 // tests/test_gpu_probe.py holds the adversarial exactness cases).

@@ -1,31 +1,38 @@
 // fwd_int4_kernel (steps a4-a9): INT4 FlashAttention forward on tcgen05 (kind::f8f6f4 on integer-exact E4M3 code
 // bytes, see fwd_int4.cuh), row-block P normaliser (reading 13).
 //
-// One CTA = one 128-row query tile of one (b,h); 28 warps, warp-specialised:
-//   warps 0-7     softmax group 0: even KV blocks; warps 0-3 own keys [0,64) of the block, warps 4-7 keys [64,128)
-//   warps 8-15    softmax group 1: odd KV blocks, same split  (two threads per query row and block)
-//   warps 16-23   drain: 2 threads per query row (D/2 channels each): online-softmax bookkeeping (m, l, alpha, beta),
-//                 P~V block -> fp32 O registers, epilogue O/l
-//   warp 24       TMEM allocator, then scale loader (Ks[j] * 2^18 log2e/sqrt(D) and Vs[g][:] -> shared rings)
-//   warp 25       TMA producer  : Q tile once, K tiles (4-stage ring) and V^T tiles (3-stage ring)
-//   warp 26       MMA issuer 2  : P~V (P codes x V codes, both from shared memory, TMEM accumulators)
-//   warp 27       MMA issuer 1  : S = Q K^T (codes x codes, exact, TMEM)
+// One CTA = one 128-row query tile of one (b,h); 16 warps, warp-specialised, ONE THREAD PER QUERY ROW in every
+// element-wise role (the tcgen05.ld 32x32b shape gives a thread its whole row, so no row reduction crosses threads):
+//   warps 0-3     softmax group 0: even KV blocks.  The thread reads the 128 accumulators of its row of S into
+//                 registers with one wait, releases the S buffer at once, and then works from registers only:
+//                 key scales + block row max, exp2 / row sum / codes, codes -> shared-memory P tile
+//   warps 4-7     softmax group 1: odd KV blocks, same code
+//   warps 8-11    drain: online-softmax bookkeeping (m, l, alpha, beta), P~V block -> fp32 O registers, epilogue O/l
+//   warp 12       TMEM allocator
+//   warp 13       TMA producer  : Q tile once, K tiles (4-stage ring) and V^T tiles (3-stage ring); with them the key
+//                 scales of the block and Vs[g][:] as 512-byte bulk copies into 8-deep shared rings
+//   warp 14       MMA issuer 2  : P~V (P codes x V codes, both from shared memory, TMEM accumulators)
+//   warp 15       MMA issuer 1  : S = Q K^T (codes x codes, exact, TMEM)
 // With the row-block normaliser the codes of block j depend only on block j, so the two softmax groups work on
-// different blocks concurrently and the running max lives in the drain threads.
+// different blocks concurrently and the running max lives in the drain threads.  Each SM sub-partition hosts one warp
+// of each softmax group, one drain warp and one service warp; the exponentials (16 per clock and SM) are the busiest
+// pipe, and the two softmax warps of a sub-partition keep it fed in turn: while one is in its load / scale / max phase
+// the other is in its exp2 phase.
 // Template switches (PAPER.md:L190 granularity; all parity-tested against the same oracle flags):
-//   QKG = 1   per-token Q/K scales (the paper's setting).  Two passes over the half row of S in tensor memory in
-//             16-column chunks: pass 1 multiplies by the key scales, writes t back over S and takes the block row max
-//             (exchanged with the partner thread through shared memory); pass 2 reads t: exp2 / row sum / codes.
-//   QKG = 128 one Q scale per query tile and one K scale per KV block: pass 1 is a bare max over the raw accumulators
-//             (no multiply, no write-back, no key-scale ring); the scalar folds into the exp2 argument of pass 2.
+//   QKG = 1   per-token Q/K scales (the paper's setting): t = S * Ks_j in registers, block row max, e = t * Qs_i - ref
+//   QKG = 128 one Q scale per query tile and one K scale per KV block: bare max over the raw accumulators (no multiply,
+//             no key-scale ring); the scalar folds into the exp2 argument.
 //   VSC = 0   one V scale per (128-token group, channel) (reading 11): drain = multiply + fma per element pair
 //   VSC = 1   one V scale per 128-token group: the scalar folds into beta, drain = one fma per element pair.
+//   SM = 1    smoothing (f2): t = S * Ks_j * Qs_i + kc_j with the per-key rank-1 correction, mean(V) added in the epilogue
 // TMEM (512 columns): S[2] at 0/128 and four half-width (D/2 channels) P~V accumulators of 64 columns at 256 (block
 // parity x channel half), so that the P~V MMAs run a block ahead of the drain instead of alternating with it.  The u8 P
-// codes go to four shared-memory tiles (128-byte swizzle, A operand from shared memory), so an S buffer is released as
-// soon as pass 2 has read it (S(j+2) is issued before P~V(j), hiding the MMA latency).
+// codes go to four shared-memory tiles (128-byte swizzle, A operand from shared memory).
 // The per-block drain is forced by the method: beta (row, block) and Vs (channel, block) change every KV block
 // (PAPER.md:L157 online softmax, L190 per-group V scales), so P~V cannot accumulate across blocks in tensor memory.
+// Keys >= N (ragged last block): the softmax thread first overwrites those columns of its S row with -inf in tensor
+// memory (a rolled loop, executed once per CTA), so the common path carries no mask; the padded key scales are 1
+// (written by prepare_qk / pad_ks into the workspace copy KsP [BH, npad] the bulk copies read).
 #pragma once
 #include <cmath>
 #include <cstdio>
@@ -36,15 +43,15 @@ namespace rotattn {
 
 // Warp roles.  Within an SM sub-partition the scheduler favours the highest warp id among the eligible warps, so the
 // latency-critical single-thread roles (MMA issue, TMA) get the highest ids and the throughput roles the lowest.
-constexpr int kWarpScale = 24, kWarpTma = 25, kWarpMmaPV = 26, kWarpMmaS = 27;
+constexpr int kWarpDrain = 8, kWarpAlloc = 12, kWarpTma = 13, kWarpMmaPV = 14, kWarpMmaS = 15;
 constexpr int K_STAGES = 4;
 constexpr int V_STAGES = 3;
 constexpr int P_SLOTS = 4;       // P-code tiles in shared memory (A operand of the P~V MMA)
 constexpr int PV_BUFS = 4;       // half-width (D/2 channel) P~V accumulators in rotation: buffer 2 * (j & 1) + h
 constexpr int AB_RING = 8;
-constexpr int KS_RING = 4;
-constexpr int VS_RING = 4;
-static_assert(K_STAGES == 4 && P_SLOTS == 4 && PV_BUFS == 4 && V_STAGES <= P_SLOTS && KS_RING == VS_RING, "ring sizes are tied together by the shared completion barriers");
+constexpr int KS_RING = 8;       // key-scale blocks in flight (bulk copies issued with the K tiles, released by the softmax threads)
+constexpr int VS_RING = 8;
+static_assert(K_STAGES == 4 && P_SLOTS == 4 && PV_BUFS == 4 && V_STAGES <= P_SLOTS, "ring sizes are tied together by the shared completion barriers");
 
 template <int D>
 struct SmemInt4 {
@@ -59,72 +66,22 @@ struct SmemInt4 {
   static constexpr int OFF_KS = OFF_P + P_SLOTS * P_BYTES;            // float [KS_RING][128]
   static constexpr int OFF_KC = OFF_KS + KS_RING * 128 * 4;           // float [KS_RING][128]  smoothing: per-key correction
   static constexpr int OFF_VS = OFF_KC + KS_RING * 128 * 4;           // float [VS_RING][D]
-  static constexpr int OFF_AB = OFF_VS + VS_RING * D * 4;             // float [AB_RING][3][128]: block max, half-row sums of the two key halves
-  static constexpr int OFF_MX = OFF_AB + AB_RING * 3 * 128 * 4;       // float [2 groups][2 parities][2 halves][128]
-  static constexpr int OFF_BAR = OFF_MX + 2 * 2 * 2 * 128 * 4;        // mbarriers
+  static constexpr int OFF_AB = OFF_VS + VS_RING * D * 4;             // float [AB_RING][2][128]: block max, block row sum
+  static constexpr int OFF_BAR = OFF_AB + AB_RING * 2 * 128 * 4;      // mbarriers
   static constexpr int NBAR = 1 + 2 * K_STAGES + V_STAGES + 2 + 2 * P_SLOTS + 2 * PV_BUFS + AB_RING + 2 * KS_RING + 2 * VS_RING;
   static constexpr int OFF_TMEM = OFF_BAR + NBAR * 8;
   static constexpr int TOTAL = OFF_TMEM + 16;
 };
-
-// ---- per-chunk element-wise work of the softmax threads (16 S columns of one query row) -------------------------
-// Pass 1.  SCALE (per-token Q/K scales): t = S * (Ks_j * 2^18 log2e/sqrt(D)) (the query scale Qs_i > 0 is applied after
-// the max), returned for the write-back over S so that pass 2 needs neither the key scales nor the mask.
-// !SCALE (one K scale per block): bare max over the raw accumulators.  Keys >= N are masked to -inf.
-// BIAS (smoothing): t = S * Ks_j * Qs_i + kc_j, the per-key rank-1 correction mean(Q) . K'_j in the log2 domain.
-template <bool SCALE, bool BIAS, bool MASK>
-__device__ __forceinline__ void chunk_scale_max(const uint32_t (&v)[16], const float2* ks2, const float2* kc2, float2 qs2,
-                                                int nvalid_rel, uint32_t (&t)[16], float& mx0, float& mx1) {
-#pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    float2 t2 = make_float2(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1]));
-    if (SCALE) t2 = fmul2(t2, ks2[i]);
-    if (BIAS) t2 = ffma2(t2, qs2, kc2[i]);
-    if (MASK) {
-      if (2 * i >= nvalid_rel) t2.x = -INFINITY;
-      if (2 * i + 1 >= nvalid_rel) t2.y = -INFINITY;
-    }
-    if (i & 1) mx1 = fmax3(mx1, t2.x, t2.y); else mx0 = fmax3(mx0, t2.x, t2.y);
-    if (SCALE) {
-      t[2 * i] = __float_as_uint(t2.x);
-      t[2 * i + 1] = __float_as_uint(t2.y);
-    }
-  }
-}
-
-// Pass 2: LEVELS * P^ = exp2(t * f - mt + log2(LEVELS)); codes u = rne(LEVELS * P^) taken from the low byte of
-// (LEVELS * P^) + 1.5 * 2^23 (Eq.12 L166-168 with the fixed scale 15 / Eq.11 L161 with 7); four codes per 32-bit word.
-// MASK (only when pass 1 did not write -inf back): keys >= N get exp2(-inf) = 0.
-template <bool MASK>
-__device__ __forceinline__ void chunk_exp(const uint32_t (&t)[16], float2 qs2, float2 nref2, int nvalid_rel, float2& ls0,
-                                          float2& ls1, uint32_t (&pw)[4]) {
-  const float2 magic2 = make_float2(12582912.f, 12582912.f);
-#pragma unroll
-  for (int g = 0; g < 4; ++g) {
-    float2 e0 = ffma2(make_float2(__uint_as_float(t[4 * g]), __uint_as_float(t[4 * g + 1])), qs2, nref2);
-    float2 e1 = ffma2(make_float2(__uint_as_float(t[4 * g + 2]), __uint_as_float(t[4 * g + 3])), qs2, nref2);
-    if (MASK) {
-      if (4 * g >= nvalid_rel) e0.x = -INFINITY;
-      if (4 * g + 1 >= nvalid_rel) e0.y = -INFINITY;
-      if (4 * g + 2 >= nvalid_rel) e1.x = -INFINITY;
-      if (4 * g + 3 >= nvalid_rel) e1.y = -INFINITY;
-    }
-    const float2 p0 = make_float2(ex2_approx(e0.x), ex2_approx(e0.y));
-    const float2 p1 = make_float2(ex2_approx(e1.x), ex2_approx(e1.y));
-    ls0 = fadd2(ls0, p0);
-    ls1 = fadd2(ls1, p1);
-    const float2 f0 = fadd2(p0, magic2), f1 = fadd2(p1, magic2);
-    const uint32_t lo = __byte_perm(__float_as_uint(f0.x), __float_as_uint(f0.y), 0x0040);
-    const uint32_t hi = __byte_perm(__float_as_uint(f1.x), __float_as_uint(f1.y), 0x0040);
-    pw[g] = __byte_perm(lo, hi, 0x5410);
-  }
-}
 
 template <int D, int P_MODE, int QKG, int VSC, int SM, bool DEBUG>
 __global__ void __launch_bounds__(kFwdThreads, 1)
 fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                 const __grid_constant__ CUtensorMap tmV, const FwdInt4Args a) {
   using L = SmemInt4<D>;
+  // Per-token variants: the softmax warps of a sub-partition alternate in the exp2 phase (token) and give 8 registers
+  // per thread to the drain (measured on cfg 2: 5.15 -> 4.98 ms; the per-block variants are faster without either).
+  constexpr bool TOKEN = QKG == 1;
+  constexpr int kRegSoftmax = QKG == 1 ? 152 : 160, kRegDrain = (65536 - 128 * 24 - 256 * kRegSoftmax) / 128;
   extern __shared__ __align__(1024) uint8_t smem[];      // no static shared memory in this kernel: base is 1024-aligned
   uint8_t* sQ = smem + L::OFF_Q;
   uint8_t* sK = smem + L::OFF_K;
@@ -134,22 +91,21 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   float* sKc = (float*)(smem + L::OFF_KC);
   float* sVs = (float*)(smem + L::OFF_VS);
   float* sAB = (float*)(smem + L::OFF_AB);
-  float* sMx = (float*)(smem + L::OFF_MX);
   uint64_t* bars = (uint64_t*)(smem + L::OFF_BAR);
   uint64_t* q_full = bars;
   uint64_t* k_full = q_full + 1;              // [K_STAGES] TMA -> MMA
   uint64_t* v_full = k_full + K_STAGES;       // [V_STAGES] TMA -> MMA
   uint64_t* s_done = v_full + V_STAGES;       // [K_STAGES] S(m) complete: -> softmax group m & 1 (S ready), -> TMA (K stage free)
-  uint64_t* s_empty = s_done + K_STAGES;      // [2] softmax group -> MMA (count 256): S buffer has been read
-  uint64_t* p_full = s_empty + 2;             // [P_SLOTS] softmax group -> MMA (count 256)
+  uint64_t* s_empty = s_done + K_STAGES;      // [2] softmax group -> MMA (count 128): S buffer is in registers
+  uint64_t* p_full = s_empty + 2;             // [P_SLOTS] softmax group -> MMA (count 128)
   uint64_t* pv_done = p_full + P_SLOTS;       // [P_SLOTS] both halves of P~V(j) complete: -> softmax (P slot free), TMA (V stage free)
-  uint64_t* pvh_done = pv_done + P_SLOTS;    // [PV_BUFS] half k = 2j+h of P~V complete -> drain warps of channel half h
+  uint64_t* pvh_done = pv_done + P_SLOTS;     // [PV_BUFS] half k = 2j+h of P~V complete -> drain
   uint64_t* pvh_empty = pvh_done + PV_BUFS;   // [PV_BUFS] drain -> MMA (count 128): half buffer is in registers
-  uint64_t* ab_full = pvh_empty + PV_BUFS;    // [AB_RING] softmax -> drain (count 256)
-  uint64_t* ks_full = ab_full + AB_RING;      // [KS_RING] loader -> softmax (count 32)
-  uint64_t* ks_empty = ks_full + KS_RING;     // [KS_RING] softmax -> loader (count 256)
-  uint64_t* vs_full = ks_empty + KS_RING;     // [VS_RING] loader -> drain (count 32)
-  uint64_t* vs_empty = vs_full + VS_RING;     // [VS_RING] drain -> loader (count 256)
+  uint64_t* ab_full = pvh_empty + PV_BUFS;    // [AB_RING] softmax -> drain (count 128)
+  uint64_t* ks_full = ab_full + AB_RING;      // [KS_RING] bulk copy of the key scales of a block -> softmax
+  uint64_t* ks_empty = ks_full + KS_RING;     // [KS_RING] softmax -> TMA producer (count 128)
+  uint64_t* vs_full = ks_empty + KS_RING;     // [VS_RING] bulk copy of Vs[g][:] -> drain
+  uint64_t* vs_empty = vs_full + VS_RING;     // [VS_RING] drain -> TMA producer (count 128)
   uint32_t* tmem_slot = (uint32_t*)(smem + L::OFF_TMEM);
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);   // warp-uniform (kept in a uniform register)
@@ -164,24 +120,24 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     mbar_init(q_full, 1);
     for (int i = 0; i < K_STAGES; ++i) { mbar_init(&k_full[i], 1); mbar_init(&s_done[i], 1); }
     for (int i = 0; i < V_STAGES; ++i) mbar_init(&v_full[i], 1);
-    for (int i = 0; i < 2; ++i) mbar_init(&s_empty[i], 256);
-    for (int i = 0; i < P_SLOTS; ++i) mbar_init(&p_full[i], 256);
+    for (int i = 0; i < 2; ++i) mbar_init(&s_empty[i], 128);
+    for (int i = 0; i < P_SLOTS; ++i) mbar_init(&p_full[i], 128);
     for (int i = 0; i < P_SLOTS; ++i) mbar_init(&pv_done[i], 1);
     for (int i = 0; i < PV_BUFS; ++i) { mbar_init(&pvh_done[i], 1); mbar_init(&pvh_empty[i], 128); }
-    for (int i = 0; i < AB_RING; ++i) mbar_init(&ab_full[i], 256);
-    for (int i = 0; i < KS_RING; ++i) { mbar_init(&ks_full[i], 32); mbar_init(&ks_empty[i], 256); }
-    for (int i = 0; i < VS_RING; ++i) { mbar_init(&vs_full[i], 32); mbar_init(&vs_empty[i], 256); }
+    for (int i = 0; i < AB_RING; ++i) mbar_init(&ab_full[i], 128);
+    for (int i = 0; i < KS_RING; ++i) { mbar_init(&ks_full[i], 1); mbar_init(&ks_empty[i], 128); }
+    for (int i = 0; i < VS_RING; ++i) { mbar_init(&vs_full[i], 1); mbar_init(&vs_empty[i], 128); }
     fence_mbar_init();
   }
-  if (warp == kWarpScale) tmem_alloc(tmem_slot, 512);
+  if (warp == kWarpAlloc) tmem_alloc(tmem_slot, 512);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
   constexpr uint32_t TM_S = 0, TM_PV = 256;                 // S[2] x 128 | PV half buffers [4] x 64
 
-  // register pool of the CTA = 896 x 72; after redistribution 128 x 24 + 512 x 72 + 256 x 96 = 64512 (exactly the pool)
-  if (warp >= 24) {
+  // register pool of the CTA = 512 x 128; after redistribution 128 x 24 + 256 x kRegSoftmax + 128 x kRegDrain = 65536
+  if (warp >= kWarpAlloc) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
     // The single-thread roles keep warp-uniform control flow (every lane waits; one elected lane issues), so that the
     // TMA / MMA operands stay in uniform registers.
@@ -203,6 +159,16 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tma_load_3d(sK + s * L::K_BYTES, &tmK, &k_full[s], 0, m * kTile, bh);
           }
           __syncwarp();
+          if (QKG == 1) {                                                     // key scales of block m (and the smoothing correction)
+            const int rg = m % KS_RING;
+            mbar_wait_hint(&ks_empty[rg], ((m / KS_RING) & 1) ^ 1);
+            if (elect_one()) {
+              mbar_arrive_expect_tx(&ks_full[rg], SM ? 1024 : 512);
+              bulk_load(smem_u32(sKs + rg * 128), a.KsP + (size_t)bh * a.npad + m * kTile, 512, smem_u32(&ks_full[rg]));
+              if (SM) bulk_load(smem_u32(sKc + rg * 128), a.KcP + (size_t)bh * a.npad + m * kTile, 512, smem_u32(&ks_full[rg]));
+            }
+            __syncwarp();
+          }
         }
         if (j >= 0) {
           const int s = j % V_STAGES;
@@ -212,6 +178,15 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tma_load_3d(sV + s * L::V_BYTES, &tmV, &v_full[s], j * kTile, 0, bh);
           }
           __syncwarp();
+          if (VSC == 0) {                                                     // V scales of group j
+            const int rg = j % VS_RING;
+            mbar_wait_hint(&vs_empty[rg], ((j / VS_RING) & 1) ^ 1);
+            if (elect_one()) {
+              mbar_arrive_expect_tx(&vs_full[rg], D * 4);
+              bulk_load(smem_u32(sVs + rg * D), a.Vs + ((size_t)bh * nblk + j) * D, D * 4, smem_u32(&vs_full[rg]));
+            }
+            __syncwarp();
+          }
         }
       }
     } else if (warp == kWarpMmaS) {
@@ -253,181 +228,166 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 #pragma unroll
             for (int k = 0; k < 4; ++k)
               mma_ss<MmaKind::F8F6F4>(tmem_base + TM_PV + buf * 64, pd + 2 * k, vd + 2 * k, idesc_pv, k != 0);
-            tc_commit(&pvh_done[buf]);                                   // -> drain warps of this channel half
+            tc_commit(&pvh_done[buf]);                                   // -> drain
             if (h == 1) tc_commit(&pv_done[slot]);                        // -> softmax (P slot free), TMA (V stage free)
           }
           __syncwarp();
         }
       }
-    } else {
-      // ---------------------------------------------------------------- scale loader: Ks_j * 2^18 log2e/sqrt(D), Vs[g][:]
-      const float* ksrc = a.Ks + (size_t)bh * a.N;
-      const float* vsrc = a.Vs + (size_t)bh * nblk * D;
-      if (QKG == 1 || VSC == 0) {
-        for (int j = 0; j < nblk; ++j) {
-          const int s = j % KS_RING;
-          float kv[4], vv[D / 32];
-          if (QKG == 1) {
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-              const int kj = j * kTile + i * 32 + lane;
-              kv[i] = (kj < a.N) ? ksrc[kj] * a.scale_log2 : 0.f;
-            }
-          }
-          if (VSC == 0) {
-#pragma unroll
-            for (int i = 0; i < D / 32; ++i) vv[i] = vsrc[(size_t)j * D + i * 32 + lane];
-          }
-          if (QKG == 1) {
-            mbar_wait_hint(&ks_empty[s], ((j / KS_RING) & 1) ^ 1);
-#pragma unroll
-            for (int i = 0; i < 4; ++i) sKs[s * 128 + i * 32 + lane] = kv[i];
-            if (SM) {                                    // per-key correction of the smoothing path (this warp has 24 registers:
-#pragma unroll                                          //  one value in flight at a time)
-              for (int i = 0; i < 4; ++i) {
-                const int kj = j * kTile + i * 32 + lane;
-                sKc[s * 128 + i * 32 + lane] = (kj < a.N) ? a.KcP[(size_t)bh * a.npad + kj] : -INFINITY;   // keys >= N: masked by the bias
-              }
-            }
-            mbar_arrive(&ks_full[s]);
-          }
-          if (VSC == 0) {
-            mbar_wait_hint(&vs_empty[s], ((j / VS_RING) & 1) ^ 1);
-#pragma unroll
-            for (int i = 0; i < D / 32; ++i) sVs[s * D + i * 32 + lane] = vv[i];
-            mbar_arrive(&vs_full[s]);
-          }
-        }
-      }
     }
-  } else if (warp < 16) {
+  } else if (warp < kWarpDrain) {
     // ------------------------------------------------------------------ softmax groups: 0 = even blocks, 1 = odd blocks
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegSoftmax));
     constexpr float LOG2_LEVELS = P_MODE == ROTATTN_P_ASYM15 ? 3.9068905956085187f : 2.8073549220576042f;
-    const int g = warp >> 3;                         // group index = S buffer index
-    const int h = (warp >> 2) & 1;                   // which 64 keys of the block
+    const int g = warp >> 2;                         // group index = S buffer index
     const int r = (warp & 3) * 32 + lane;
     const int row = q0 + r;
-    const int cb = 64 * h;
     const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
-    // Per-token: f = Qs_i (the key scales carry 2^18 log2e/sqrt(D)); qs >= 1e-30 keeps (-inf) * qs well defined for masked
-    // keys; an all-zero query row still gives s == 0 everywhere.  QKG = 128: f = Qs_tile * Ks_block * 2^18 log2e/sqrt(D).
+    // Per-token: f = Qs_i * 2^18 log2e/sqrt(D); f >= 1e-30 keeps (-inf) * f well defined for masked keys; an all-zero
+    // query row still gives s == 0 everywhere.  QKG = 128: f = Qs_tile * Ks_block * 2^18 log2e/sqrt(D).
     float fq;
-    if (QKG == 1) fq = (row < a.N) ? fmaxf(a.Qs[(size_t)bh * a.N + row], 1e-30f) : 1e-30f;
+    if (QKG == 1) fq = (row < a.N) ? fmaxf(a.Qs[(size_t)bh * a.N + row] * a.scale_log2, 1e-30f) : 1e-30f;
     else fq = a.Qs[(size_t)bh * nblk + qtile] * a.scale_log2;
     const float* ksg = a.Ks + (size_t)bh * nblk;           // QKG = 128 only
-    const uint32_t s_addr = tmem_base + lane_off + TM_S + g * 128 + cb;
-    const int pair_bar = 1 + 4 * g + (warp & 3);     // named barrier of the two warps that share these 32 rows
+    const uint32_t s_addr = tmem_base + lane_off + TM_S + g * 128;
+    const uint32_t p_row0 = smem_u32(sP) + r * 128;        // 16-byte chunk q of row r lives at chunk q ^ (r & 7)
+    const uint32_t swz = (uint32_t)(r & 7) << 4;
+    const int tok_mine = 1 + 4 * g + (warp & 3), tok_other = 1 + 4 * (g ^ 1) + (warp & 3);
+    if (TOKEN && g == 1) bar_arrive(tok_other, 64);        // group 0 takes the first turn
     for (int j = g; j < nblk; j += 2) {
-      const int n = j >> 1;
       const int ring = j % KS_RING, slot = j % P_SLOTS, abslot = j % AB_RING;
-      const float2* ks2 = reinterpret_cast<const float2*>(sKs + ring * 128 + cb);
-      const int nvalid = min(kTile, a.N - j * kTile) - cb;   // valid keys of this half; < 64 only on the ragged last block
-      const bool ragged = nvalid < 64;
+      const int nvalid = a.N - j * kTile;                  // < 128 only on the ragged last block
       float qs = fq;
       if (QKG != 1) qs *= ksg[j];
       const float2 qs2 = make_float2(qs, qs);
       if (QKG == 1) mbar_wait(&ks_full[ring], (j / KS_RING) & 1);
       mbar_wait(&s_done[j % K_STAGES], (j / K_STAGES) & 1);
       tc_fence_after();
-      uint32_t va[16], vb[16], tt[16];
-      // ---- pass 1: t = S * ks (written back over S), block row max over this half
-      float mx0 = -INFINITY, mx1 = -INFINITY;
-      tmem_ld16(s_addr, va);
-      auto pass1 = [&](auto masked) {                    // one branch per block on the ragged case, not one per chunk
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
+      if (nvalid < kTile) {                                // keys >= N: -inf over their accumulators (once per CTA)
+#pragma unroll 1
+        for (int c = nvalid >> 4; c < 8; ++c) {
+          uint32_t v[16];
+          tmem_ld16(s_addr + c * 16, v);
           tmem_wait_ld();
-          uint32_t(&cur)[16] = (c & 1) ? vb : va;
-          uint32_t(&nxt)[16] = (c & 1) ? va : vb;
-          if (c < 3) tmem_ld16(s_addr + (c + 1) * 16, nxt);
-          else if (QKG != 1) tmem_ld16(s_addr, nxt);       // chunk 0 again for pass 2, in flight across the max exchange
-          if (DEBUG) {
 #pragma unroll
-            for (int i = 0; i < 16; ++i)
-              a.S_dump[(size_t)r * a.npad + j * kTile + cb + c * 16 + i] = (int32_t)(__uint_as_float(cur[i]) * kAccScale);
-          }
-          chunk_scale_max<QKG == 1, SM != 0, decltype(masked)::value>(cur, ks2 + c * 8, ks2 + c * 8 + (L::OFF_KC - L::OFF_KS) / 8, qs2, nvalid - c * 16, tt, mx0, mx1);
-          if (QKG == 1) tmem_st16(s_addr + c * 16, tt);
+          for (int i = 0; i < 16; ++i) v[i] = (c * 16 + i >= nvalid) ? 0xff800000u : v[i];
+          tmem_st16(s_addr + c * 16, v);
         }
-      };
-      // smoothing: the additive per-key term is -inf for keys >= N, so the ragged block needs no separate code
-      if (ragged && !SM) pass1(std::true_type{}); else pass1(std::false_type{});
-      float tmax = fmaxf(mx0, mx1);
-      float* mxbuf = sMx + ((g * 2 + (n & 1)) * 2) * 128;
-      mxbuf[h * 128 + r] = tmax;
-      if (QKG == 1) {
-        mbar_arrive(&ks_empty[ring]);
         tmem_wait_st();
-        tmem_ld16(s_addr, va);                           // chunk 0 of t, in flight across the max exchange
       }
-      bar_sync(pair_bar, 64);
-      tmax = fmaxf(tmax, mxbuf[(h ^ 1) * 128 + r]);
-      const float mt = SM ? tmax : qs * tmax;            // block row max of s * log2e (smoothing: Qs_i is already in t)
+      uint32_t u[4][32];                                   // the row of S: accumulator * 2^-18 as fp32
+#pragma unroll
+      for (int c = 0; c < 4; ++c) tmem_ld32(s_addr + c * 32, u[c]);
+      tmem_wait_ld();
+      tc_fence_before();
+      mbar_arrive(&s_empty[g]);                            // S(j+2) may be issued: this thread works from registers now
+      if (DEBUG) {
+#pragma unroll
+        for (int i = 0; i < 128; ++i)
+          a.S_dump[(size_t)r * a.npad + j * kTile + i] = (int32_t)(__uint_as_float(u[i >> 5][i & 31]) * kAccScale);
+      }
+      // ---- t = S * ks (per-token), block row max
+      float mx0 = -INFINITY, mx1 = -INFINITY;
+      {
+        const float4* ks4 = reinterpret_cast<const float4*>(sKs + ring * 128);
+        const float4* kc4 = reinterpret_cast<const float4*>(sKc + ring * 128);
+#pragma unroll
+        for (int c = 0; c < 32; ++c) {
+          uint32_t* w = &u[c >> 3][(c & 7) * 4];
+          float2 t0 = make_float2(__uint_as_float(w[0]), __uint_as_float(w[1]));
+          float2 t1 = make_float2(__uint_as_float(w[2]), __uint_as_float(w[3]));
+          if (QKG == 1) {
+            const float4 k = ks4[c];
+            t0 = fmul2(t0, make_float2(k.x, k.y));
+            t1 = fmul2(t1, make_float2(k.z, k.w));
+          }
+          if (SM) {
+            const float4 k = kc4[c];
+            t0 = ffma2(t0, qs2, make_float2(k.x, k.y));
+            t1 = ffma2(t1, qs2, make_float2(k.z, k.w));
+          }
+          mx0 = fmax3(mx0, t0.x, t0.y);
+          mx1 = fmax3(mx1, t1.x, t1.y);
+          if (QKG == 1 || SM) {
+            w[0] = __float_as_uint(t0.x); w[1] = __float_as_uint(t0.y);
+            w[2] = __float_as_uint(t1.x); w[3] = __float_as_uint(t1.y);
+          }
+        }
+      }
+      if (QKG == 1) mbar_arrive(&ks_empty[ring]);
+      const float tmax = fmaxf(mx0, mx1);
+      const float mt = SM ? tmax : qs * tmax;              // block row max of s * log2e (smoothing: Qs_i is already in t)
       const float nref = LOG2_LEVELS - mt;
       const float2 nref2 = make_float2(nref, nref);
+      const float2 es2 = SM ? make_float2(1.f, 1.f) : qs2;
       mbar_wait(&pv_done[slot], ((j / P_SLOTS) & 1) ^ 1);            // P~V(j-4) has consumed this P slot
-      // ---- pass 2: LEVELS * P^, row sum, codes -> u8 P tile slot
+      // The two softmax warps of an SM sub-partition (one of each group) take turns in the exp2 phase (a token passed
+      // through two named barriers): one of them feeds the exp2 unit while the other is in its load / scale / max phase,
+      // instead of both running the same phase side by side and leaving the unit idle in between.
+      if (TOKEN) bar_sync(tok_mine, 64);
+      // ---- LEVELS * P^ = exp2(t * f - mt + log2(LEVELS)); codes u = rne(LEVELS * P^) taken from the low byte of
+      // (LEVELS * P^) + 1.5 * 2^23 (Eq.12 L166-168 with the fixed scale 15 / Eq.11 L161 with 7); four codes per 32-bit word
       float2 ls0 = make_float2(0.f, 0.f), ls1 = make_float2(0.f, 0.f);
-      uint8_t* p_row = sP + slot * L::P_BYTES + r * 128;             // 16-byte chunk q of row r lives at chunk q ^ (r & 7)
-      auto pass2 = [&](auto masked) {
+      const float2 magic2 = make_float2(12582912.f, 12582912.f);
+      const uint32_t p_row = p_row0 + slot * L::P_BYTES;
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-          tmem_wait_ld();
-          uint32_t(&cur)[16] = (c & 1) ? vb : va;
-          uint32_t(&nxt)[16] = (c & 1) ? va : vb;
-          if (c < 3) tmem_ld16(s_addr + (c + 1) * 16, nxt);
-          else { tc_fence_before(); mbar_arrive(&s_empty[g]); }          // this thread is done with the S buffer
-          uint32_t pw[4];
-          chunk_exp<decltype(masked)::value>(cur, SM ? make_float2(1.f, 1.f) : qs2, nref2, nvalid - c * 16, ls0, ls1, pw);
-          if (DEBUG) {
+      for (int q = 0; q < 8; ++q) {
+        uint32_t pw[4];
 #pragma unroll
-            for (int q = 0; q < 4; ++q) *reinterpret_cast<uint32_t*>(a.P_dump + (size_t)r * a.npad + j * kTile + cb + c * 16 + q * 4) = pw[q];
-          }
-          *reinterpret_cast<uint4*>(p_row + (((4 * h + c) ^ (r & 7)) << 4)) = make_uint4(pw[0], pw[1], pw[2], pw[3]);
+        for (int x = 0; x < 4; ++x) {
+          const uint32_t* w = &u[q >> 1][(q & 1) * 16 + x * 4];
+          const float2 e0 = ffma2(make_float2(__uint_as_float(w[0]), __uint_as_float(w[1])), es2, nref2);
+          const float2 e1 = ffma2(make_float2(__uint_as_float(w[2]), __uint_as_float(w[3])), es2, nref2);
+          const float2 p0 = make_float2(ex2_approx(e0.x), ex2_approx(e0.y));
+          const float2 p1 = make_float2(ex2_approx(e1.x), ex2_approx(e1.y));
+          ls0 = fadd2(ls0, p0);
+          ls1 = fadd2(ls1, p1);
+          const float2 f0 = fadd2(p0, magic2), f1 = fadd2(p1, magic2);
+          const uint32_t lo = __byte_perm(__float_as_uint(f0.x), __float_as_uint(f0.y), 0x0040);
+          const uint32_t hi = __byte_perm(__float_as_uint(f1.x), __float_as_uint(f1.y), 0x0040);
+          pw[x] = __byte_perm(lo, hi, 0x5410);
         }
-      };
-      if (QKG != 1 && ragged) pass2(std::true_type{}); else pass2(std::false_type{});
-      if (h == 0) sAB[(abslot * 3) * 128 + r] = mt;
-      sAB[(abslot * 3 + 1 + h) * 128 + r] = (ls0.x + ls0.y) + (ls1.x + ls1.y);
+        if (DEBUG) {
+#pragma unroll
+          for (int x = 0; x < 4; ++x) *reinterpret_cast<uint32_t*>(a.P_dump + (size_t)r * a.npad + j * kTile + q * 16 + x * 4) = pw[x];
+        }
+        sts_u32x4(p_row + (((uint32_t)q << 4) ^ swz), pw[0], pw[1], pw[2], pw[3]);
+      }
+      if (TOKEN) bar_arrive(tok_other, 64);
+      sAB[(abslot * 2) * 128 + r] = mt;
+      sAB[(abslot * 2 + 1) * 128 + r] = (ls0.x + ls0.y) + (ls1.x + ls1.y);
       fence_proxy_async_smem();                          // P codes (generic-proxy stores) -> visible to the MMA (async proxy)
       mbar_arrive(&p_full[slot]);
       mbar_arrive(&ab_full[abslot]);
     }
   } else {
-    // ------------------------------------------------------------------ drain: 2 threads per query row of O
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 96;");
-    constexpr int DH = D / 2;                      // channels per thread
-    const int h = (warp >> 2) & 1, r = (warp & 3) * 32 + lane;
+    // ------------------------------------------------------------------ drain: one thread per query row of O
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegDrain));
+    constexpr int DH = D / 2;                      // channels per P~V half buffer
+    const int r = (warp & 3) * 32 + lane;
     const int row = q0 + r;
     const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
-    float2 o2[DH / 2];
+    float2 o2[D / 2];
 #pragma unroll
-    for (int d = 0; d < DH / 2; ++d) o2[d] = make_float2(0.f, 0.f);
+    for (int d = 0; d < D / 2; ++d) o2[d] = make_float2(0.f, 0.f);
     // Online softmax bookkeeping (L157) with a lazily updated reference max: O and l are kept relative to m_ref, which
     // only moves when a block max exceeds it by more than 2^8 (fp32 has the headroom), so the common path is
-    // O += beta * pv * Vs with beta = exp2(mt - m_ref) and no rescale of the 64 accumulators.
+    // O += beta * pv * Vs with beta = exp2(mt - m_ref) and no rescale of the accumulators.
     constexpr float kLazy = 8.f;
     float m_ref = -INFINITY, l_run = 0.f;
     const float* vsg = a.Vs + (size_t)bh * nblk;             // VSC = 1 only
     for (int j = 0; j < nblk; ++j) {
       const int abslot = j % AB_RING;
       mbar_wait(&ab_full[abslot], (j / AB_RING) & 1);
-      const float mt = sAB[(abslot * 3) * 128 + r];
-      const float bsum = sAB[(abslot * 3 + 1) * 128 + r] + sAB[(abslot * 3 + 2) * 128 + r];
+      const float mt = sAB[(abslot * 2) * 128 + r];
+      const float bsum = sAB[(abslot * 2 + 1) * 128 + r];
       const int vring = j % VS_RING;
-      const int buf = 2 * (j & 1) + h;
-      const uint32_t pv_addr = tmem_base + lane_off + TM_PV + buf * 64;
-      if (VSC == 0) mbar_wait(&vs_full[vring], (j / VS_RING) & 1);
-      mbar_wait(&pvh_done[buf], (j >> 1) & 1);
-      tc_fence_after();
-      uint32_t va[16], vb[16];
-      tmem_ld16(pv_addr, va);                                          // in flight across the bookkeeping below
       if (__any_sync(0xffffffffu, mt > m_ref + kLazy)) {               // rare after the first blocks (warp-uniform branch)
         const float m_new = (mt > m_ref + kLazy) ? mt : m_ref;
         const float alpha = ex2_approx(m_ref - m_new);                 // first block: exp2(-inf) = 0; unchanged rows: 1
         const float2 a2 = make_float2(alpha, alpha);
 #pragma unroll
-        for (int d = 0; d < DH / 2; ++d) o2[d] = fmul2(o2[d], a2);
+        for (int d = 0; d < D / 2; ++d) o2[d] = fmul2(o2[d], a2);
         l_run *= alpha;
         m_ref = m_new;
       }
@@ -436,36 +396,54 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       float cf = beta * kAccScale;                                     // undoes the 2^-18 of the E4M3 code products
       if (VSC != 0) cf *= vsg[j];
       const float2 c2 = make_float2(cf, cf);
-      const float2* vsb2 = reinterpret_cast<const float2*>(sVs + vring * D + h * DH);
+      if (VSC == 0) mbar_wait(&vs_full[vring], (j / VS_RING) & 1);
 #pragma unroll
-      for (int cc = 0; cc < DH / 16; ++cc) {
-        tmem_wait_ld();
-        uint32_t(&cur)[16] = (cc & 1) ? vb : va;
-        uint32_t(&nxt)[16] = (cc & 1) ? va : vb;
-        if (cc + 1 < DH / 16) tmem_ld16(pv_addr + (cc + 1) * 16, nxt);
-        else { tc_fence_before(); mbar_arrive(&pvh_empty[buf]); }      // this half-width accumulator is in registers now
-        if (DEBUG) {
-          if (a.PV_dump) {
+      for (int h = 0; h < 2; ++h) {
+        const int buf = 2 * (j & 1) + h;
+        const uint32_t pv_addr = tmem_base + lane_off + TM_PV + buf * 64;
+        const float4* vsb4 = reinterpret_cast<const float4*>(sVs + vring * D + h * DH);
+        mbar_wait(&pvh_done[buf], (j >> 1) & 1);
+        tc_fence_after();
+        uint32_t va[16], vb[16];
+        tmem_ld16(pv_addr, va);
 #pragma unroll
-            for (int i = 0; i < 16; ++i)
-              a.PV_dump[((size_t)j * kTile + r) * D + h * DH + cc * 16 + i] = (int32_t)(__uint_as_float(cur[i]) * kAccScale);
+        for (int cc = 0; cc < DH / 16; ++cc) {
+          tmem_wait_ld();
+          uint32_t(&cur)[16] = (cc & 1) ? vb : va;
+          uint32_t(&nxt)[16] = (cc & 1) ? va : vb;
+          if (cc + 1 < DH / 16) tmem_ld16(pv_addr + (cc + 1) * 16, nxt);
+          else { tc_fence_before(); mbar_arrive(&pvh_empty[buf]); }      // this half-width accumulator is in registers now
+          if (DEBUG) {
+            if (a.PV_dump) {
+#pragma unroll
+              for (int i = 0; i < 16; ++i)
+                a.PV_dump[((size_t)j * kTile + r) * D + h * DH + cc * 16 + i] = (int32_t)(__uint_as_float(cur[i]) * kAccScale);
+            }
           }
-        }
 #pragma unroll
-        for (int d = 0; d < 8; ++d) {
-          float2 y = make_float2(__uint_as_float(cur[2 * d]), __uint_as_float(cur[2 * d + 1]));
-          if (VSC == 0) y = fmul2(y, vsb2[cc * 8 + d]);
-          o2[cc * 8 + d] = ffma2(y, c2, o2[cc * 8 + d]);               // O += beta * pv * Vs[g][d]
+          for (int d = 0; d < 4; ++d) {
+            float2 y0 = make_float2(__uint_as_float(cur[4 * d]), __uint_as_float(cur[4 * d + 1]));
+            float2 y1 = make_float2(__uint_as_float(cur[4 * d + 2]), __uint_as_float(cur[4 * d + 3]));
+            if (VSC == 0) {
+              const float4 s = vsb4[cc * 4 + d];
+              y0 = fmul2(y0, make_float2(s.x, s.y));
+              y1 = fmul2(y1, make_float2(s.z, s.w));
+            }
+            float2& oa = o2[h * (DH / 2) + cc * 8 + 2 * d];
+            float2& ob = o2[h * (DH / 2) + cc * 8 + 2 * d + 1];
+            oa = ffma2(y0, c2, oa);                                      // O += beta * pv * Vs[g][d]
+            ob = ffma2(y1, c2, ob);
+          }
         }
       }
       if (VSC == 0) mbar_arrive(&vs_empty[vring]);
     }
     const float inv_l = 1.f / l_run;
     if (row < a.N) {
-      __half* dst = (DEBUG ? a.O + (size_t)r * D : a.O + ((size_t)bh * a.N + row) * D) + h * DH;
-      const float2* mv2 = reinterpret_cast<const float2*>(a.means + ((size_t)bh * 3 + 2) * D + h * DH);   // smoothing: mean of V
+      __half* dst = DEBUG ? a.O + (size_t)r * D : a.O + ((size_t)bh * a.N + row) * D;
+      const float2* mv2 = reinterpret_cast<const float2*>(a.means + ((size_t)bh * 3 + 2) * D);   // smoothing: mean of V
 #pragma unroll
-      for (int d = 0; d < DH; d += 8) {
+      for (int d = 0; d < D; d += 8) {
         __half2 hh[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
@@ -479,7 +457,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == kWarpScale) tmem_dealloc(tmem_base, 512);
+  if (warp == kWarpAlloc) tmem_dealloc(tmem_base, 512);
 }
 
 
@@ -493,8 +471,8 @@ int launch_one(const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& 
   if (!checked) {
     cudaFuncAttributes fa;
     ROTATTN_CUDA_TRY(cudaFuncGetAttributes(&fa, kern));
-    if (fa.numRegs != 72) {
-      set_error_text("fwd_int4_kernel: unexpected register allocation (setmaxnreg pool assumes 72 registers per thread)");
+    if (fa.numRegs != 128) {
+      set_error_text("fwd_int4_kernel: unexpected register allocation (setmaxnreg pool assumes 128 registers per thread)");
       return ROTATTN_ERR_UNSUPPORTED;
     }
     ROTATTN_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));

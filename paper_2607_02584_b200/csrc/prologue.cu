@@ -305,6 +305,13 @@ __global__ void __launch_bounds__(256, 2) prepare_qk_kernel(const PrepArgs a) {
   };
 
   if (QKG == 1) {
+    // padded tail of the workspace copies [BH, npad] (read block-wise by fwd_int4's bulk copies): scale 1, correction 0
+    if (blockIdx.x == 0 && warp == 0) {
+      for (int n = a.N + lane; n < a.npad; n += 32) {
+        if (a.KsP) a.KsP[bh * a.npad + n] = 1.f;
+        if (MODE == PREP_QUANT_SMOOTH && a.KcP) a.KcP[bh * a.npad + n] = 0.f;
+      }
+    }
     // blockIdx.y = (b,h); the warps of the grid's x dimension stride over that head's tokens, TOK consecutive ones at a time
     const int nstride = gridDim.x * WPB * TOK;
     for (int n0 = (blockIdx.x * WPB + warp) * TOK; n0 < a.N; n0 += nstride) {
@@ -639,7 +646,7 @@ __global__ void pad_ks_kernel(const float* __restrict__ Ks, float* __restrict__ 
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= BH * npad) return;
   const int n = (int)(i % npad);
-  KsP[i] = n < N ? Ks[(i / npad) * N + n] : 0.f;
+  KsP[i] = n < N ? Ks[(i / npad) * N + n] : 1.f;       // keys >= N: fwd_int4 masks their accumulators with -inf, the scale must be finite and > 0
 }
 
 int launch_unpack_qk(const rotattn_params& p, const uint8_t* X4, int8_t* X8, cudaStream_t st) {

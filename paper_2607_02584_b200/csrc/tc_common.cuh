@@ -279,6 +279,7 @@ __device__ __forceinline__ bool elect_one() {
 
 // named barrier over a subset of the CTA's warps
 __device__ __forceinline__ void bar_sync(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
+__device__ __forceinline__ void bar_arrive(int id, int nthreads) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
 
 // ------------------------------------------------------------------------------------------------
 // Host: tensor maps (driver entry point fetched through the runtime; no link against libcuda)
