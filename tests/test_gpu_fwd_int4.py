@@ -42,6 +42,21 @@ def test_d128_ragged_multi_tile(base):
             ph.check_tile(res, po, 0, h, qt, inputs=(pq['q_codes'], pq['q_scale'], pq['k_codes'], pq['k_scale'], vc, vs))
 
 
+@pytest.mark.parametrize('grid', [(1, 9, 11), (1, 10, 13), (3, 5, 17), (2, 8, 8)])
+@pytest.mark.parametrize('qk_group', [1, 128])
+def test_ragged_edge_blocks(grid, qk_group):
+    """Degenerate shapes of the masked last KV block: a single ragged block (N = 99: the odd-block softmax group has no work),
+    a last block with 2 valid keys (N = 130: every 16-column chunk of it is masked in tensor memory), N = 255 (one key short of
+    two full blocks) and an exact multiple (N = 128: no masked column at all)."""
+    w = syn.small_variant(syn.WAN_1_3B, grid, H=2)
+    q, k, v = syn.gen_all(w)
+    res, po, tab = ph.run_path(w, q, k, v, rot_mode=orc.ROT_HALF, qk_group=qk_group)
+    for h in range(w.H):
+        pq, vc, vs, _ = ph.check_prologue_head(po, tab, res, q[0, h], k[0, h], v[0, h], 0, h)
+        for qt in range(-(-w.N // 128)):
+            ph.check_tile(res, po, 0, h, qt, inputs=(pq['q_codes'], pq['q_scale'], pq['k_codes'], pq['k_scale'], vc, vs))
+
+
 @pytest.mark.parametrize('qk_group,v_scale', F1)
 @pytest.mark.parametrize('p_mode', [orc.P_ASYM15, orc.P_SYM7])
 def test_granularity_variants_tiny_and_ragged(qk_group, v_scale, p_mode):

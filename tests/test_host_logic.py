@@ -132,8 +132,11 @@ def test_compute_entry_points_fail_loudly_without_gpu():
 
 
 def test_attention_kernels_fit_the_instruction_cache():
-    """past 32 KB of SASS (2048 instructions of 16 bytes) fwd_int4 falls off an instruction-cache
-    cliff (34 KB: 9.2 ms against 5.9 ms for the same work).  Every shipped non-debug variant must stay below it."""
+    """the 28-warp fwd_int4 of round 1 fell off an instruction-cache cliff once its code passed 32 KB
+    (34 KB: 9.2 ms against 5.9 ms for the same work).  The one-thread-per-row kernel is 33-39 KB in total, but what runs in
+    steady state (the block loops of the softmax, drain and service warps) is about 18 KB, and the measured hit rate of the
+    38 KB headline variant is 99.94 % (profiles/r2_int4_path_ncu_full.md: sm__icc_request_hit_rate).  Guard: no shipped
+    non-debug variant above 40 KB, so that growth beyond what was measured is noticed."""
     import shutil
     import subprocess
     if shutil.which('cuobjdump') is None:
@@ -154,4 +157,4 @@ def test_attention_kernels_fit_the_instruction_cache():
                 counts[name] += 1
     assert len(counts) == 20, len(counts)            # 2 head dims x (8 granularity / P-mode variants + 2 smoothing variants)
     worst = max(counts.values())
-    assert worst * 16 <= 33 * 1024, {k: v for k, v in counts.items() if v * 16 > 33 * 1024}
+    assert worst * 16 <= 40 * 1024, {k: v for k, v in counts.items() if v * 16 > 40 * 1024}
