@@ -17,7 +17,9 @@
 // different blocks concurrently and the running max lives in the drain threads.  Each SM sub-partition hosts one warp
 // of each softmax group, one drain warp and one service warp; the exponentials (16 per clock and SM) are the busiest
 // pipe, and the two softmax warps of a sub-partition keep it fed in turn: while one is in its load / scale / max phase
-// the other is in its exp2 phase.
+// the other is in its exp2 phase (per-token variants: enforced by a token passed through two named barriers per pair of
+// warps; the per-block variants, whose non-exp2 phase is short, run free - DESIGN.md section 12 has the measurements).
+// Registers: 512 x 128 at launch, redistributed by setmaxnreg to 24 (service) / 152-160 (softmax) / 168-184 (drain).
 // Template switches (PAPER.md:L190 granularity; all parity-tested against the same oracle flags):
 //   QKG = 1   per-token Q/K scales (the paper's setting): t = S * Ks_j in registers, block row max, e = t * Qs_i - ref
 //   QKG = 128 one Q scale per query tile and one K scale per KV block: bare max over the raw accumulators (no multiply,
