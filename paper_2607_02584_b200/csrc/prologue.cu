@@ -1,7 +1,7 @@
 // Prologue kernels (HBM-bound): prepare_qk (a1+a2), quant_v (a3), the smoothing pre-pass (f2) and the unpack helpers.
 // Code-producing arithmetic is fp32 with one rounding per operation (__fmul_rn/__fadd_rn/__fsub_rn/__fdiv_rn,
 // never contracted) so that the INT4 codes are reproducible bit for bit ("bit-exact prologue").
-#include "common.cuh"
+#include "tc_common.cuh"     // packed fp32x2 arithmetic (mul.rn / add.rn per lane: the same roundings as the scalar forms)
 
 namespace rotattn {
 
@@ -75,17 +75,37 @@ struct PrepLane {
   }
 };
 
+// Sum of two packed products with one rounding per operation: ptxas contracts mul.rn.f32x2 + add.rn.f32x2 into one FFMA2
+// (a single rounding, which would change codes at rounding ties), but it never contracts the scalar add.rn.f32, so the
+// products are packed and the additions scalar.
+__device__ __forceinline__ float2 add2_rn(float2 a, float2 b) { return make_float2(__fadd_rn(a.x, b.x), __fadd_rn(a.y, b.y)); }
+
+// (t,h,w) of a token index walked with a constant stride: two 32-bit divisions once, then additions with carries
+// (the stride is decomposed once; every component of it is smaller than its axis, so one carry per axis suffices).
+struct PosWalk {
+  int pt, ph, pw, st, sh, sw;
+  __device__ __forceinline__ void init(int n0, int stride, int gh, int gw) {
+    pw = n0 % gw; int pr = n0 / gw; ph = pr % gh; pt = pr / gh;
+    sw = stride % gw; int sr = stride / gw; sh = sr % gh; st = sr / gh;
+  }
+  __device__ __forceinline__ void advance(int gh, int gw) {
+    pw += sw;
+    int c = pw >= gw; pw -= c ? gw : 0;
+    ph += sh + c;
+    c = ph >= gh; ph -= c ? gh : 0;
+    pt += st + c;
+  }
+};
+
 // y = x (M R) for kPrepTok consecutive tokens of one head (Q and K): RoPE through the coefficient table (INTERLEAVED is
 // merged into it, Eq.7), then HALF (Eq.8, partner exchange through shared memory) or FULL (the paper's
 // "Full" baseline L208: D x D Hadamard as an in-register / shuffle butterfly) in the same register pass.
 template <int D, int ROT>
 __device__ __forceinline__ void prep_compute_y(const PrepArgs& a, const PrepLane<D, ROT>& ln, float* ybuf_warp, long long head0,
-                                               int n0, int lane, __half (&hx)[kPrepTok][2][D / 32],
+                                               int n0, int pt, int ph, int pw, int lane, __half (&hx)[kPrepTok][2][D / 32],
                                                float (&y)[kPrepTok][2][D / 32]) {
   constexpr int CPL = D / 32, PPL = CPL / 2, TOK = kPrepTok;
-  // (t,h,w) of the first token by two 32-bit divisions; the following ones by carry propagation
-  int pw = n0 % a.gw, pr = n0 / a.gw;
-  int ph = pr % a.gh, pt = pr / a.gh;
+  // (pt, ph, pw) = (t,h,w) of token n0 (row-major, reading 4); the following tokens by carry propagation
   // ---- load phase: TOK tokens x (Q, K) + their coefficient rows, all independent
   float4 A[TOK][PPL];
   const bool full = n0 + TOK <= a.N;                     // warp-uniform: no per-token guards on the common path
@@ -126,9 +146,12 @@ __device__ __forceinline__ void prep_compute_y(const PrepArgs& a, const PrepLane
     for (int m = 0; m < 2; ++m)
 #pragma unroll
       for (int i = 0; i < PPL; ++i) {
-        float x0 = __half2float(hx[t][m][2 * i]), x1 = __half2float(hx[t][m][2 * i + 1]);
-        y[t][m][2 * i]     = __fadd_rn(__fmul_rn(x0, A[t][i].x), __fmul_rn(x1, A[t][i].z));
-        y[t][m][2 * i + 1] = __fadd_rn(__fmul_rn(x0, A[t][i].y), __fmul_rn(x1, A[t][i].w));
+        const float x0 = __half2float(hx[t][m][2 * i]), x1 = __half2float(hx[t][m][2 * i + 1]);
+        // (y0, y1) = x0 (a, b) + x1 (c, d): two packed multiplies and two adds, every operation rounded once
+        const float2 r = add2_rn(fmul2(make_float2(x0, x0), make_float2(A[t][i].x, A[t][i].y)),
+                                 fmul2(make_float2(x1, x1), make_float2(A[t][i].z, A[t][i].w)));
+        y[t][m][2 * i] = r.x;
+        y[t][m][2 * i + 1] = r.y;
       }
   if (ROT == ROTATTN_ROT_HALF) {
     float (*yb)[2][D] = reinterpret_cast<float (*)[2][D]>(ybuf_warp);
@@ -145,9 +168,12 @@ __device__ __forceinline__ void prep_compute_y(const PrepArgs& a, const PrepLane
 #pragma unroll
       for (int m = 0; m < 2; ++m)
 #pragma unroll
-        for (int j = 0; j < CPL; ++j) {
-          const float other = yb[t][m][ln.partner[j]];
-          y[t][m][j] = __fadd_rn(__fmul_rn(y[t][m][j], ln.ca[j]), __fmul_rn(other, ln.cb[j]));   // fp32 addition commutes exactly
+        for (int j = 0; j < CPL; j += 2) {
+          const float2 other = make_float2(yb[t][m][ln.partner[j]], yb[t][m][ln.partner[j + 1]]);
+          const float2 r = add2_rn(fmul2(make_float2(y[t][m][j], y[t][m][j + 1]), make_float2(ln.ca[j], ln.ca[j + 1])),
+                                   fmul2(other, make_float2(ln.cb[j], ln.cb[j + 1])));             // fp32 addition commutes exactly
+          y[t][m][j] = r.x;
+          y[t][m][j + 1] = r.y;
         }
     __syncwarp();
   }
@@ -184,31 +210,37 @@ __device__ __forceinline__ void prep_store_token(const PrepArgs& a, int m, long 
                                                  float inv) {
   constexpr int CPL = D / 32;
   // code = rne(y * inv) is in [-7,7] without clamping (|y| <= amax and inv = rn(7/amax) give |y*inv| < 7.5).
-  // fs = q + 1.5*2^23 holds the two's-complement code in its low byte, fa = |q| + 1.5*2^23 the magnitude.
-  uint32_t fs[CPL], fa[CPL], yb[CPL];
-#pragma unroll
-  for (int j = 0; j < CPL; ++j) {
-    const float q = __fmul_rn(yq[j], inv);
-    fs[j] = __float_as_uint(__fadd_rn(q, 12582912.f));
-    fa[j] = __float_as_uint(__fadd_rn(fabsf(q), 12582912.f));
-    yb[j] = __float_as_uint(q);
-  }
+  // fs = q + 1.5*2^23 holds the two's-complement code in its low byte.
   if (CPL == 4) {
-    const uint32_t n01 = (fs[0] & 0xFu) | ((fs[1] << 4) & 0xF0u), n23 = (fs[2] & 0xFu) | ((fs[3] << 4) & 0xF0u);
-    *reinterpret_cast<uint16_t*>(a.X4[m] + tok * (D / 2) + lane * 2) = (uint16_t)__byte_perm(n01, n23, 0x0040);
+    const float2 inv2 = make_float2(inv, inv), magic2 = make_float2(12582912.f, 12582912.f);
+    const float2 f01 = add2_rn(fmul2(make_float2(yq[0], yq[1]), inv2), magic2);
+    const float2 f23 = add2_rn(fmul2(make_float2(yq[2], yq[3]), inv2), magic2);
+    // w = the four codes as two's-complement bytes
+    const uint32_t w = __byte_perm(__byte_perm(__float_as_uint(f01.x), __float_as_uint(f01.y), 0x0040),
+                                   __byte_perm(__float_as_uint(f23.x), __float_as_uint(f23.y), 0x0040), 0x5410);
+    // packed nibbles: byte 0 = (c0 & 0xF) | (c1 & 0xF) << 4, byte 2 = the same of (c2, c3)
+    const uint32_t nib = (w & 0x000F000Fu) | ((w >> 4) & 0x00F000F0u);
+    *reinterpret_cast<uint16_t*>(a.X4[m] + tok * (D / 2) + lane * 2) = (uint16_t)__byte_perm(nib, nib, 0x0020);
+    if (a.X8[m]) {
+      // sign-magnitude operand bytes (code_byte): per byte |c| = (c ^ s) + t with t = the sign bit and s = 0xFF t
+      // (|c| <= 7: no carry leaves a byte); a zero code has no sign bit, so there is no -0 byte.
+      const uint32_t t = (w >> 7) & 0x01010101u;
+      const uint32_t mag = (w ^ (t * 0xFFu)) + t;
+      *reinterpret_cast<uint32_t*>(a.X8[m] + tok * kQKRowBytes + lane * 4) = mag | (w & 0x80808080u);
+    }
   } else {
+    uint32_t fs[CPL], fa[CPL], yb[CPL];
+#pragma unroll
+    for (int j = 0; j < CPL; ++j) {
+      const float q = __fmul_rn(yq[j], inv);
+      fs[j] = __float_as_uint(__fadd_rn(q, 12582912.f));
+      fa[j] = __float_as_uint(__fadd_rn(fabsf(q), 12582912.f));       // |q| + 1.5*2^23: the magnitude in the low byte
+      yb[j] = __float_as_uint(q);
+    }
     a.X4[m][tok * (D / 2) + lane] = (uint8_t)((fs[0] & 0xFu) | ((fs[1] << 4) & 0xF0u));
-  }
-  if (a.X8[m]) {
-    // sign-magnitude operand bytes (code_byte): magnitude bytes | sign bits of q, the sign only where the magnitude byte
-    // is non-zero (a zero code has q = +-0 or |q| < 0.5: no -0 byte)
-    int8_t* dst = a.X8[m] + tok * kQKRowBytes;
-    if (CPL == 4) {
-      const uint32_t mag = __byte_perm(__byte_perm(fa[0], fa[1], 0x0040), __byte_perm(fa[2], fa[3], 0x0040), 0x5410);
-      const uint32_t sgn = __byte_perm(__byte_perm(yb[0], yb[1], 0x0073), __byte_perm(yb[2], yb[3], 0x0073), 0x5410);
-      const uint32_t nz = ((mag + 0x7F7F7F7Fu) & 0x80808080u);     // 0x80 in every byte whose magnitude is non-zero
-      *reinterpret_cast<uint32_t*>(dst + lane * 4) = mag | (sgn & nz);
-    } else {
+    if (a.X8[m]) {
+      // magnitude bytes | sign bits of q, the sign only where the magnitude byte is non-zero (no -0 byte)
+      int8_t* dst = a.X8[m] + tok * kQKRowBytes;
       const uint32_t mag = __byte_perm(fa[0], fa[1], 0x0040) & 0xFFFFu;
       const uint32_t sgn = __byte_perm(yb[0], yb[1], 0x0073) & 0xFFFFu;
       const uint32_t nz = ((mag + 0x7F7Fu) & 0x8080u);
@@ -264,8 +296,10 @@ __global__ void __launch_bounds__(256, 2) prepare_qk_kernel(const PrepArgs a) {
     for (int i = threadIdx.x; i < 2 * D; i += blockDim.x) ssum[i] = 0;
     __syncthreads();
     const int nstride = gridDim.x * WPB * TOK;
-    for (int n0 = (blockIdx.x * WPB + warp) * TOK; n0 < a.N; n0 += nstride) {
-      prep_compute_y<D, ROT>(a, ln, &ybuf[ROT == ROTATTN_ROT_HALF ? warp : 0][0][0][0], head0, n0, lane, hx, y);
+    PosWalk pos;
+    pos.init((blockIdx.x * WPB + warp) * TOK, nstride, a.gh, a.gw);
+    for (int n0 = (blockIdx.x * WPB + warp) * TOK; n0 < a.N; n0 += nstride, pos.advance(a.gh, a.gw)) {
+      prep_compute_y<D, ROT>(a, ln, &ybuf[ROT == ROTATTN_ROT_HALF ? warp : 0][0][0][0], head0, n0, pos.pt, pos.ph, pos.pw, lane, hx, y);
 #pragma unroll
       for (int t = 0; t < TOK; ++t)
         if (n0 + t < a.N) {
@@ -314,8 +348,10 @@ __global__ void __launch_bounds__(256, 2) prepare_qk_kernel(const PrepArgs a) {
     }
     // blockIdx.y = (b,h); the warps of the grid's x dimension stride over that head's tokens, TOK consecutive ones at a time
     const int nstride = gridDim.x * WPB * TOK;
-    for (int n0 = (blockIdx.x * WPB + warp) * TOK; n0 < a.N; n0 += nstride) {
-      prep_compute_y<D, ROT>(a, ln, &ybuf[ROT == ROTATTN_ROT_HALF ? warp : 0][0][0][0], head0, n0, lane, hx, y);
+    PosWalk pos;
+    pos.init((blockIdx.x * WPB + warp) * TOK, nstride, a.gh, a.gw);
+    for (int n0 = (blockIdx.x * WPB + warp) * TOK; n0 < a.N; n0 += nstride, pos.advance(a.gh, a.gw)) {
+      prep_compute_y<D, ROT>(a, ln, &ybuf[ROT == ROTATTN_ROT_HALF ? warp : 0][0][0][0], head0, n0, pos.pt, pos.ph, pos.pw, lane, hx, y);
       if (a.X16[0]) {                                     // fp16 copies for the FP16 path: y before smoothing
 #pragma unroll
         for (int t = 0; t < TOK; ++t)
@@ -372,10 +408,12 @@ __global__ void __launch_bounds__(256, 2) prepare_qk_kernel(const PrepArgs a) {
     for (int g = blockIdx.x; g < a.nG; g += gridDim.x) {
       const int gbase = g * kTile + warp * (kTile / WPB);
       float am0 = 0.f, am1 = 0.f;
-      for (int i = 0; i < kTile / WPB / TOK; ++i) {
+      PosWalk pos;
+      pos.init(gbase, TOK, a.gh, a.gw);
+      for (int i = 0; i < kTile / WPB / TOK; ++i, pos.advance(a.gh, a.gw)) {
         const int n0 = gbase + i * TOK;
         if (n0 >= a.N) break;
-        prep_compute_y<D, ROT>(a, ln, &ybuf[ROT == ROTATTN_ROT_HALF ? warp : 0][0][0][0], head0, n0, lane, hx, y);
+        prep_compute_y<D, ROT>(a, ln, &ybuf[ROT == ROTATTN_ROT_HALF ? warp : 0][0][0][0], head0, n0, pos.pt, pos.ph, pos.pw, lane, hx, y);
 #pragma unroll
         for (int t = 0; t < TOK; ++t)
           if (n0 + t < a.N) {
@@ -398,10 +436,11 @@ __global__ void __launch_bounds__(256, 2) prepare_qk_kernel(const PrepArgs a) {
         a.Xs[0][bh * a.nG + g] = __fdiv_rn(am0, 7.0f);
         a.Xs[1][bh * a.nG + g] = __fdiv_rn(am1, 7.0f);
       }
-      for (int i = 0; i < kTile / WPB / TOK; ++i) {
+      pos.init(gbase, TOK, a.gh, a.gw);
+      for (int i = 0; i < kTile / WPB / TOK; ++i, pos.advance(a.gh, a.gw)) {
         const int n0 = gbase + i * TOK;
         if (n0 >= a.N) break;
-        prep_compute_y<D, ROT>(a, ln, &ybuf[ROT == ROTATTN_ROT_HALF ? warp : 0][0][0][0], head0, n0, lane, hx, y);
+        prep_compute_y<D, ROT>(a, ln, &ybuf[ROT == ROTATTN_ROT_HALF ? warp : 0][0][0][0], head0, n0, pos.pt, pos.ph, pos.pw, lane, hx, y);
 #pragma unroll
         for (int t = 0; t < TOK; ++t) {
           if (n0 + t >= a.N) break;
