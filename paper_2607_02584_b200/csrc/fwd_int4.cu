@@ -1,6 +1,5 @@
 // rotattn_fwd_int4 / rotattn_fwd_int4_debug: host side of the INT4 attention kernels (argument checks, workspace
-// copies, tensor maps, variant dispatch).  The kernels are in fwd_int4_kernel.cuh (ROWBLOCK normaliser) and
-// fwd_int4_sync.cu (RUNNING normaliser).
+// copies, tensor maps, variant dispatch).  The kernel is in fwd_int4_kernel.cuh (ROWBLOCK and RUNNING normalisers).
 #include <cmath>
 #include <cstdio>
 #include "fwd_int4.cuh"
@@ -52,7 +51,6 @@ int fwd_int4_common(const rotattn_params* p, const uint8_t* Q4, const float* Qs,
   a.N = p->N; a.nblk = nblk; a.npad = ws.npad; a.dbg_bh = bh; a.dbg_qtile = q_tile;
   a.scale_log2 = (float)(1.4426950408889634 / std::sqrt((double)p->D) * (double)kAccScale);   // S arrives as acc * 2^-18
   dim3 grid(debug ? 1 : nblk, debug ? 1 : (head_sel ? n_sel : BH));
-  if (p->p_norm == ROTATTN_NORM_RUNNING) return launch_fwd_int4_sync(*p, tq, tk, tv, a, grid, debug, cs);
   if (debug) return launch_fwd_int4_debug(*p, tq, tk, tv, a, grid, cs);
   return p->D == 128 ? launch_fwd_int4_d128(*p, tq, tk, tv, a, grid, cs) : launch_fwd_int4_d64(*p, tq, tk, tv, a, grid, cs);
 }

@@ -1,11 +1,9 @@
-// Shared declarations of the INT4 attention kernels (fwd_int4_kernel.cuh: ROWBLOCK normaliser, block-independent
-// softmax; fwd_int4_sync.cu: RUNNING normaliser, softmax serialised over KV blocks).
+// Shared declarations of the INT4 attention kernel (fwd_int4_kernel.cuh: ROWBLOCK and RUNNING normalisers).
 #pragma once
 #include "tc_common.cuh"
 
 namespace rotattn {
 
-constexpr int kInt4Threads = 640;      // fwd_int4_sync_kernel
 constexpr int kFwdThreads = 512;       // fwd_int4_kernel
 // The widened operands are E4M3 bytes that encode code * 2^-9 (see prologue.cu: code_byte), so both tensor products
 // arrive in tensor memory as fp32 values  integer_accumulator * 2^-18  (exact: |acc| <= 13440 < 2^24;
@@ -35,15 +33,11 @@ __device__ __forceinline__ float ex2_approx(float x) {
   return y;
 }
 
-// ROWBLOCK kernel, one translation unit per head dimension / debug flavour (parallel compilation)
+// one translation unit per head dimension / debug flavour (parallel compilation)
 int launch_fwd_int4_d128(const rotattn_params& p, const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv,
                          const FwdInt4Args& a, dim3 grid, cudaStream_t cs);
 int launch_fwd_int4_d64(const rotattn_params& p, const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv,
                         const FwdInt4Args& a, dim3 grid, cudaStream_t cs);
 int launch_fwd_int4_debug(const rotattn_params& p, const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv,
                           const FwdInt4Args& a, dim3 grid, cudaStream_t cs);
-// RUNNING-normaliser kernel (fwd_int4_sync.cu)
-int launch_fwd_int4_sync(const rotattn_params& p, const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv,
-                         const FwdInt4Args& a, dim3 grid, bool debug, cudaStream_t cs);
-
 }  // namespace rotattn

@@ -53,6 +53,7 @@ constexpr int PV_BUFS = 4;       // half-width (D/2 channel) P~V accumulators in
 constexpr int AB_RING = 8;
 constexpr int KS_RING = 8;       // key-scale blocks in flight (bulk copies issued with the K tiles, released by the softmax threads)
 constexpr int VS_RING = 8;
+constexpr int RUN_RING = 4;      // p_norm = RUNNING: running row maxima handed from block j to block j + 1 (the other softmax group)
 static_assert(K_STAGES == 4 && P_SLOTS == 4 && PV_BUFS == 4 && V_STAGES <= P_SLOTS, "ring sizes are tied together by the shared completion barriers");
 
 template <int D>
@@ -69,13 +70,14 @@ struct SmemInt4 {
   static constexpr int OFF_KC = OFF_KS + KS_RING * 128 * 4;           // float [KS_RING][128]  smoothing: per-key correction
   static constexpr int OFF_VS = OFF_KC + KS_RING * 128 * 4;           // float [VS_RING][D]
   static constexpr int OFF_AB = OFF_VS + VS_RING * D * 4;             // float [AB_RING][2][128]: block max, block row sum
-  static constexpr int OFF_BAR = OFF_AB + AB_RING * 2 * 128 * 4;      // mbarriers
-  static constexpr int NBAR = 1 + 2 * K_STAGES + V_STAGES + 2 + 2 * P_SLOTS + 2 * PV_BUFS + AB_RING + 2 * KS_RING + 2 * VS_RING;
+  static constexpr int OFF_RUN = OFF_AB + AB_RING * 2 * 128 * 4;      // float [RUN_RING][128]  p_norm = RUNNING: running row max after block j
+  static constexpr int OFF_BAR = OFF_RUN + RUN_RING * 128 * 4;        // mbarriers
+  static constexpr int NBAR = 1 + 2 * K_STAGES + V_STAGES + 2 + 2 * P_SLOTS + 2 * PV_BUFS + AB_RING + 2 * KS_RING + 2 * VS_RING + RUN_RING;
   static constexpr int OFF_TMEM = OFF_BAR + NBAR * 8;
   static constexpr int TOTAL = OFF_TMEM + 16;
 };
 
-template <int D, int P_MODE, int QKG, int VSC, int SM, bool DEBUG>
+template <int D, int P_MODE, int QKG, int VSC, int SM, int PN, bool DEBUG>
 __global__ void __launch_bounds__(kFwdThreads, 1)
 fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                 const __grid_constant__ CUtensorMap tmV, const FwdInt4Args a) {
@@ -93,6 +95,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   float* sKc = (float*)(smem + L::OFF_KC);
   float* sVs = (float*)(smem + L::OFF_VS);
   float* sAB = (float*)(smem + L::OFF_AB);
+  float* sRun = (float*)(smem + L::OFF_RUN);
   uint64_t* bars = (uint64_t*)(smem + L::OFF_BAR);
   uint64_t* q_full = bars;
   uint64_t* k_full = q_full + 1;              // [K_STAGES] TMA -> MMA
@@ -108,6 +111,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   uint64_t* ks_empty = ks_full + KS_RING;     // [KS_RING] softmax -> TMA producer (count 128)
   uint64_t* vs_full = ks_empty + KS_RING;     // [VS_RING] bulk copy of Vs[g][:] -> drain
   uint64_t* vs_empty = vs_full + VS_RING;     // [VS_RING] drain -> TMA producer (count 128)
+  uint64_t* run_full = vs_empty + VS_RING;    // [RUN_RING] softmax(j) -> softmax(j + 1) (count 128): running max after block j
   uint32_t* tmem_slot = (uint32_t*)(smem + L::OFF_TMEM);
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);   // warp-uniform (kept in a uniform register)
@@ -129,6 +133,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     for (int i = 0; i < AB_RING; ++i) mbar_init(&ab_full[i], 128);
     for (int i = 0; i < KS_RING; ++i) { mbar_init(&ks_full[i], 1); mbar_init(&ks_empty[i], 128); }
     for (int i = 0; i < VS_RING; ++i) { mbar_init(&vs_full[i], 1); mbar_init(&vs_empty[i], 128); }
+    for (int i = 0; i < RUN_RING; ++i) mbar_init(&run_full[i], 128);
     fence_mbar_init();
   }
   if (warp == kWarpAlloc) tmem_alloc(tmem_slot, 512);
@@ -318,7 +323,19 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       }
       if (QKG == 1) mbar_arrive(&ks_empty[ring]);
       const float tmax = fmaxf(mx0, mx1);
-      const float mt = SM ? tmax : qs * tmax;              // block row max of s * log2e (smoothing: Qs_i is already in t)
+      float mt = SM ? tmax : qs * tmax;                    // block row max of s * log2e (smoothing: Qs_i is already in t)
+      if (PN == ROTATTN_NORM_RUNNING) {
+        // Codes relative to the running max (SURVEY 8c reading 13, alternative): block j needs the maximum over blocks
+        // <= j.  Block j - 1 belongs to the other softmax group, whose thread of the same row publishes its running max
+        // right after its own max pass, so only the max passes are serialised, not the exp2 phases.  The drain needs no
+        // change: it receives the normaliser of the block, whatever its definition.
+        if (j > 0) {
+          mbar_wait(&run_full[(j - 1) % RUN_RING], ((j - 1) / RUN_RING) & 1);
+          mt = fmaxf(mt, sRun[((j - 1) % RUN_RING) * 128 + r]);
+        }
+        sRun[(j % RUN_RING) * 128 + r] = mt;               // slot reuse: block j + 4 starts after block j + 3, which read block j + 2, ...
+        mbar_arrive(&run_full[j % RUN_RING]);
+      }
       const float nref = LOG2_LEVELS - mt;
       const float2 nref2 = make_float2(nref, nref);
       const float2 es2 = SM ? make_float2(1.f, 1.f) : qs2;
@@ -464,11 +481,11 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 
 
 // ---- host side: variant dispatch for one (D, DEBUG) flavour -------------------------------------------------------
-template <int D, int P_MODE, int QKG, int VSC, int SM, bool DEBUG>
+template <int D, int P_MODE, int QKG, int VSC, int SM, int PN, bool DEBUG>
 int launch_one(const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv, const FwdInt4Args& a, dim3 grid,
                cudaStream_t cs) {
   constexpr int smem = SmemInt4<D>::TOTAL;
-  auto kern = fwd_int4_kernel<D, P_MODE, QKG, VSC, SM, DEBUG>;
+  auto kern = fwd_int4_kernel<D, P_MODE, QKG, VSC, SM, PN, DEBUG>;
   static int checked = 0;       // once per variant: ptxas must have allocated exactly the register pool setmaxnreg assumes
   if (!checked) {
     cudaFuncAttributes fa;
@@ -489,18 +506,21 @@ template <int D, bool DEBUG>
 int launch_variants(const rotattn_params& p, const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv,
                     const FwdInt4Args& a, dim3 grid, cudaStream_t cs) {
   const int sel = (p.p_mode == ROTATTN_P_SYM7 ? 4 : 0) | (p.qk_group == 128 ? 2 : 0) | (p.v_scale == ROTATTN_VSCALE_GROUP ? 1 : 0);
+  if (p.p_norm == ROTATTN_NORM_RUNNING)   // validated: the running normaliser comes with the paper's granularity only, without smoothing
+    return sel & 4 ? launch_one<D, ROTATTN_P_SYM7, 1, 0, 0, ROTATTN_NORM_RUNNING, DEBUG>(tq, tk, tv, a, grid, cs)
+                   : launch_one<D, ROTATTN_P_ASYM15, 1, 0, 0, ROTATTN_NORM_RUNNING, DEBUG>(tq, tk, tv, a, grid, cs);
   if (p.smooth)        // validated: smoothing comes with the paper's granularity only
-    return sel & 4 ? launch_one<D, ROTATTN_P_SYM7, 1, 0, 1, DEBUG>(tq, tk, tv, a, grid, cs)
-                   : launch_one<D, ROTATTN_P_ASYM15, 1, 0, 1, DEBUG>(tq, tk, tv, a, grid, cs);
+    return sel & 4 ? launch_one<D, ROTATTN_P_SYM7, 1, 0, 1, ROTATTN_NORM_ROWBLOCK, DEBUG>(tq, tk, tv, a, grid, cs)
+                   : launch_one<D, ROTATTN_P_ASYM15, 1, 0, 1, ROTATTN_NORM_ROWBLOCK, DEBUG>(tq, tk, tv, a, grid, cs);
   switch (sel) {
-    case 0: return launch_one<D, ROTATTN_P_ASYM15, 1, 0, 0, DEBUG>(tq, tk, tv, a, grid, cs);
-    case 1: return launch_one<D, ROTATTN_P_ASYM15, 1, 1, 0, DEBUG>(tq, tk, tv, a, grid, cs);
-    case 2: return launch_one<D, ROTATTN_P_ASYM15, 128, 0, 0, DEBUG>(tq, tk, tv, a, grid, cs);
-    case 3: return launch_one<D, ROTATTN_P_ASYM15, 128, 1, 0, DEBUG>(tq, tk, tv, a, grid, cs);
-    case 4: return launch_one<D, ROTATTN_P_SYM7, 1, 0, 0, DEBUG>(tq, tk, tv, a, grid, cs);
-    case 5: return launch_one<D, ROTATTN_P_SYM7, 1, 1, 0, DEBUG>(tq, tk, tv, a, grid, cs);
-    case 6: return launch_one<D, ROTATTN_P_SYM7, 128, 0, 0, DEBUG>(tq, tk, tv, a, grid, cs);
-    default: return launch_one<D, ROTATTN_P_SYM7, 128, 1, 0, DEBUG>(tq, tk, tv, a, grid, cs);
+    case 0: return launch_one<D, ROTATTN_P_ASYM15, 1, 0, 0, ROTATTN_NORM_ROWBLOCK, DEBUG>(tq, tk, tv, a, grid, cs);
+    case 1: return launch_one<D, ROTATTN_P_ASYM15, 1, 1, 0, ROTATTN_NORM_ROWBLOCK, DEBUG>(tq, tk, tv, a, grid, cs);
+    case 2: return launch_one<D, ROTATTN_P_ASYM15, 128, 0, 0, ROTATTN_NORM_ROWBLOCK, DEBUG>(tq, tk, tv, a, grid, cs);
+    case 3: return launch_one<D, ROTATTN_P_ASYM15, 128, 1, 0, ROTATTN_NORM_ROWBLOCK, DEBUG>(tq, tk, tv, a, grid, cs);
+    case 4: return launch_one<D, ROTATTN_P_SYM7, 1, 0, 0, ROTATTN_NORM_ROWBLOCK, DEBUG>(tq, tk, tv, a, grid, cs);
+    case 5: return launch_one<D, ROTATTN_P_SYM7, 1, 1, 0, ROTATTN_NORM_ROWBLOCK, DEBUG>(tq, tk, tv, a, grid, cs);
+    case 6: return launch_one<D, ROTATTN_P_SYM7, 128, 0, 0, ROTATTN_NORM_ROWBLOCK, DEBUG>(tq, tk, tv, a, grid, cs);
+    default: return launch_one<D, ROTATTN_P_SYM7, 128, 1, 0, ROTATTN_NORM_ROWBLOCK, DEBUG>(tq, tk, tv, a, grid, cs);
   }
 }
 

@@ -155,6 +155,6 @@ def test_attention_kernels_fit_the_instruction_cache():
                 counts[name] = 0
             elif name and re.match(r'\s+/\*[0-9a-f]{4,5}\*/', line):
                 counts[name] += 1
-    assert len(counts) == 20, len(counts)            # 2 head dims x (8 granularity / P-mode variants + 2 smoothing variants)
+    assert len(counts) == 24, len(counts)            # 2 head dims x (8 granularity / P-mode variants + 2 smoothing + 2 running-normaliser variants)
     worst = max(counts.values())
     assert worst * 16 <= 40 * 1024, {k: v for k, v in counts.items() if v * 16 > 40 * 1024}
