@@ -57,6 +57,20 @@ def test_ragged_edge_blocks(grid, qk_group):
             ph.check_tile(res, po, 0, h, qt, inputs=(pq['q_codes'], pq['q_scale'], pq['k_codes'], pq['k_scale'], vc, vs))
 
 
+@pytest.mark.parametrize('grid', [(1, 9, 11), (1, 10, 13), (3, 9, 13)])
+def test_running_normaliser_edge_blocks(grid):
+    """p_norm = RUNNING in the one-thread-per-row kernel: the running row max is handed from block j (one softmax group) to
+    block j + 1 (the other group).  One ragged block (nobody to hand to), two blocks with 2 valid keys in the second, three
+    blocks with a ragged tail."""
+    w = syn.small_variant(syn.WAN_1_3B, grid, H=2)
+    q, k, v = syn.gen_all(w)
+    res, po, tab = ph.run_path(w, q, k, v, rot_mode=orc.ROT_HALF, p_norm=orc.NORM_RUNNING)
+    for h in range(w.H):
+        pq, vc, vs, _ = ph.check_prologue_head(po, tab, res, q[0, h], k[0, h], v[0, h], 0, h)
+        for qt in range(-(-w.N // 128)):
+            ph.check_tile(res, po, 0, h, qt, inputs=(pq['q_codes'], pq['q_scale'], pq['k_codes'], pq['k_scale'], vc, vs))
+
+
 @pytest.mark.parametrize('qk_group,v_scale', F1)
 @pytest.mark.parametrize('p_mode', [orc.P_ASYM15, orc.P_SYM7])
 def test_granularity_variants_tiny_and_ragged(qk_group, v_scale, p_mode):
