@@ -372,35 +372,39 @@ __global__ void __launch_bounds__(256, 2) prepare_qk_kernel(const PrepArgs a) {
           for (int j = 0; j < CPL; ++j) v = fmaxf(v, fabsf(y[t][m][j]));
           amax[t][m] = v;
         }
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1)
-#pragma unroll
-        for (int t = 0; t < TOK; ++t)
-#pragma unroll
-          for (int m = 0; m < 2; ++m) amax[t][m] = fmaxf(amax[t][m], __shfl_xor_sync(0xffffffffu, amax[t][m], o));
-      // scale = amax / 7 and inv = 7 / amax are IEEE divisions: lane (2 t + m) computes the pair once, then broadcast
-      float my_inv = 0.f;
+      // Reduction of the TOK x 2 = 8 maxima over the 32 lanes with 9 shuffles instead of 40: at offsets 16, 8, 4 every lane
+      // keeps the half of its values that belongs to its side of the exchange and sends the other half, so that lanes
+      // [4 i, 4 i + 4) end up with the maximum of value i = 2 t + m (max is exact: the result is the same bit pattern).
+      static_assert(TOK == 4, "the transposing reduction is written for 8 values");
+      float z;
       {
-        float am = 0.f;
+        const bool h16 = lane & 16, h8 = lane & 8, h4 = lane & 4;
+        float w4[4], w2[2];
 #pragma unroll
-        for (int t = 0; t < TOK; ++t)
-#pragma unroll
-          for (int m = 0; m < 2; ++m) am = (lane == 2 * t + m) ? amax[t][m] : am;
-        if (lane < 2 * TOK) {
-          const float my_scale = __fdiv_rn(am, 7.0f);
-          my_inv = am > 0.f ? __fdiv_rn(7.0f, am) : 0.f;
-          if (n0 + (lane >> 1) < a.N) {                     // lane 2 t + m owns (token t, tensor m)
-            a.Xs[lane & 1][head0 + n0 + (lane >> 1)] = my_scale;
-            if ((lane & 1) && a.KsP) a.KsP[bh * a.npad + n0 + (lane >> 1)] = my_scale;
-          }
+        for (int k = 0; k < 4; ++k) {
+          const float lo = amax[k >> 1][k & 1], hi = amax[(k + 4) >> 1][(k + 4) & 1];
+          w4[k] = fmaxf(h16 ? hi : lo, __shfl_xor_sync(0xffffffffu, h16 ? lo : hi, 16));
         }
+#pragma unroll
+        for (int k = 0; k < 2; ++k) w2[k] = fmaxf(h8 ? w4[k + 2] : w4[k], __shfl_xor_sync(0xffffffffu, h8 ? w4[k] : w4[k + 2], 8));
+        z = fmaxf(h4 ? w2[1] : w2[0], __shfl_xor_sync(0xffffffffu, h4 ? w2[0] : w2[1], 4));
+        z = fmaxf(z, __shfl_xor_sync(0xffffffffu, z, 2));
+        z = fmaxf(z, __shfl_xor_sync(0xffffffffu, z, 1));
+      }
+      // scale = amax / 7 and inv = 7 / amax are IEEE divisions, computed by the lanes that hold the value (lane >> 2 = 2 t + m)
+      const float my_scale = __fdiv_rn(z, 7.0f);
+      const float my_inv = z > 0.f ? __fdiv_rn(7.0f, z) : 0.f;
+      if ((lane & 3) == 0 && n0 + (lane >> 3) < a.N) {    // lane 4 (2 t + m) stores for (token t, tensor m)
+        const int m = (lane >> 2) & 1;
+        a.Xs[m][head0 + n0 + (lane >> 3)] = my_scale;
+        if (m && a.KsP) a.KsP[bh * a.npad + n0 + (lane >> 3)] = my_scale;
       }
 #pragma unroll
       for (int t = 0; t < TOK; ++t) {
         if (n0 + t >= a.N) break;
 #pragma unroll
         for (int m = 0; m < 2; ++m)
-          prep_store_token<D>(a, m, head0 + n0 + t, lane, y[t][m], __shfl_sync(0xffffffffu, my_inv, 2 * t + m));
+          prep_store_token<D>(a, m, head0 + n0 + t, lane, y[t][m], __shfl_sync(0xffffffffu, my_inv, 4 * (2 * t + m)));
       }
     }
   } else {
