@@ -19,7 +19,7 @@
 // pipe, and the two softmax warps of a sub-partition keep it fed in turn: while one is in its load / scale / max phase
 // the other is in its exp2 phase (per-token variants: enforced by a token passed through two named barriers per pair of
 // warps; the per-block variants, whose non-exp2 phase is short, run free - DESIGN.md section 12 has the measurements).
-// Registers: 512 x 128 at launch, redistributed by setmaxnreg to 24 (service) / 152-160 (softmax) / 168-184 (drain).
+// Registers: 512 x 128 at launch, redistributed by setmaxnreg to 24 (service) / 152 (softmax) / 184 (drain).
 // Template switches (PAPER.md:L190 granularity; all parity-tested against the same oracle flags):
 //   QKG = 1   per-token Q/K scales (the paper's setting): t = S * Ks_j in registers, block row max, e = t * Qs_i - ref
 //   QKG = 128 one Q scale per query tile and one K scale per KV block: bare max over the raw accumulators (no multiply,
@@ -43,8 +43,7 @@
 
 namespace rotattn {
 
-// Warp roles.  Within an SM sub-partition the scheduler favours the highest warp id among the eligible warps, so the
-// latency-critical single-thread roles (MMA issue, TMA) get the highest ids and the throughput roles the lowest.
+// Warp roles (role indices; the map from physical warps to roles is in the kernel, it depends on the variant).
 constexpr int kWarpDrain = 8, kWarpAlloc = 12, kWarpTma = 13, kWarpMmaPV = 14, kWarpMmaS = 15;
 constexpr int K_STAGES = 4;
 constexpr int V_STAGES = 3;
@@ -82,10 +81,10 @@ __global__ void __launch_bounds__(kFwdThreads, 1)
 fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                 const __grid_constant__ CUtensorMap tmV, const FwdInt4Args a) {
   using L = SmemInt4<D>;
-  // Per-token variants: the softmax warps of a sub-partition alternate in the exp2 phase (token) and give 8 registers
-  // per thread to the drain (measured on cfg 2: 5.15 -> 4.98 ms; the per-block variants are faster without either).
+  // Per-token variants: the softmax warps of a sub-partition alternate in the exp2 phase (token; measured on cfg 2:
+  // 5.15 -> 4.98 ms; the per-block variants are faster without it).
   constexpr bool TOKEN = QKG == 1;
-  constexpr int kRegSoftmax = QKG == 1 ? 152 : 160, kRegDrain = (65536 - 128 * 24 - 256 * kRegSoftmax) / 128;
+  constexpr int kRegSoftmax = 152, kRegDrain = (65536 - 128 * 24 - 256 * kRegSoftmax) / 128;
   extern __shared__ __align__(1024) uint8_t smem[];      // no static shared memory in this kernel: base is 1024-aligned
   uint8_t* sQ = smem + L::OFF_Q;
   uint8_t* sK = smem + L::OFF_K;
@@ -114,7 +113,13 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   uint64_t* run_full = vs_empty + VS_RING;    // [RUN_RING] softmax(j) -> softmax(j + 1) (count 128): running max after block j
   uint32_t* tmem_slot = (uint32_t*)(smem + L::OFF_TMEM);
 
-  const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);   // warp-uniform (kept in a uniform register)
+  // Role of a warp.  Within an SM sub-partition the scheduler favours the highest warp id among the eligible warps.  The
+  // per-token variants keep the service warps on the highest ids (with them on the lowest the kernel is 22 % slower: the
+  // latency from an arrival to the MMA issue is on its critical path); the per-block variants, whose softmax warps wait
+  // less, are 2-3 % faster with the softmax warps on top (physical warps 0-3 service, 4-7 drain, 8-15 softmax).  Roles
+  // move in whole warp quads, so the TMEM lane quarter of a warp (warp % 4) is the same in both maps.
+  const int pwarp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);  // warp-uniform (kept in a uniform register)
+  const int warp = QKG == 1 ? pwarp : (pwarp < 4 ? pwarp + 12 : (pwarp < 8 ? pwarp + 4 : pwarp - 8));
   const int lane = threadIdx.x & 31;
   const int qtile = DEBUG ? a.dbg_qtile : blockIdx.x;
   const int bh = DEBUG ? a.dbg_bh : (a.head_sel ? a.head_sel[blockIdx.y] : (int)blockIdx.y);
