@@ -347,7 +347,9 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       mbar_wait(&pv_done[slot], ((j / P_SLOTS) & 1) ^ 1);            // P~V(j-4) has consumed this P slot
       // The two softmax warps of an SM sub-partition (one of each group) take turns in the exp2 phase (a token passed
       // through two named barriers): one of them feeds the exp2 unit while the other is in its load / scale / max phase,
-      // instead of both running the same phase side by side and leaving the unit idle in between.
+      // instead of both running the same phase side by side and leaving the unit idle in between.  bar.sync orders memory
+      // operations only: ptxas schedules the 64 exponent FFMA2 and the first ~19 MUFU.EX2 of the block before it, which is
+      // the best split measured (everything behind the token: +6 %).
       if (TOKEN) bar_sync(tok_mine, 64);
       // ---- LEVELS * P^ = exp2(t * f - mt + log2(LEVELS)); codes u = rne(LEVELS * P^) taken from the low byte of
       // (LEVELS * P^) + 1.5 * 2^23 (Eq.12 L166-168 with the fixed scale 15 / Eq.11 L161 with 7); four codes per 32-bit word
