@@ -176,6 +176,32 @@ int rotattn_fwd_int4(const rotattn_params* p,
                      const int32_t* head_sel, int32_t n_sel,
                      void* workspace, size_t ws_bytes, int32_t ws_state, void* stream);
 
+/* rotattn_fwd_int4 for callers that cannot supply a workspace and must not allocate one.
+ *
+ * Typical callers: a DiT serving process whose own arena took all of HBM at start-up and which forbids cudaMalloc on the
+ * request path (an allocation there synchronises the device, stalls the other streams and may fail outright), or an
+ * operator plugged into a foreign runtime through an "inputs, outputs" signature with no workspace slot.
+ *
+ * Same computation and same kernels as rotattn_fwd_int4 with ws_state = 0 (steps a4-a9, PAPER.md 4.2 L155-170): the
+ * operand copies are rebuilt from the packed Q4/K4/V4 on every call.  The workspace is a device array of
+ * ROTATTN_STATIC_WS_BYTES built into librotattn.so; every GPU that loads the library carries it until the process ends.
+ *  - Limit: rotattn_workspace_bytes(p, 1) <= ROTATTN_STATIC_WS_BYTES (roughly B*H*N <= 21 000 tokens at D = 128, e.g. one
+ *    head of a 480p video or all 12 heads of a 1 700-token clip).  Larger shapes return ROTATTN_ERR_WORKSPACE_TOO_SMALL
+ *    (text in rotattn_last_cuda_error()); split them over heads with separate per-head calls.
+ *  - smooth = 1 returns ROTATTN_ERR_UNSUPPORTED (its state lives in the prologue's workspace).
+ *  - This call allocates nothing and frees nothing: no cudaMalloc / cudaFree / allocating library routine, here or below.
+ *  - The first call on each device looks up the array's device address (cudaGetSymbolAddress, that device current) and
+ *    remembers it; make that first call during start-up, before any stream capture begins on that device.
+ *  - ALL calls on a device share the one array, and it keeps what the previous call left.  Each call rewrites every byte
+ *    it later reads, so stale contents are harmless and nothing needs clearing - but two calls that overlap on the GPU
+ *    (different streams, no ordering between them) race on it and corrupt each other.  Calls on one stream are safe.
+ * Arguments as for rotattn_fwd_int4 (caller-owned device pointers; O 16-byte aligned; head_sel may be NULL). */
+#define ROTATTN_STATIC_WS_BYTES (8u << 20)
+int rotattn_fwd_int4_static(const rotattn_params* p,
+                            const uint8_t* Q4, const float* Qs, const uint8_t* K4, const float* Ks,
+                            const uint8_t* V4, const float* Vs, void* O,
+                            const int32_t* head_sel, int32_t n_sel, void* stream);
+
 /* Step a10: FP16 FlashAttention forward, the fallback precision and the speed baseline (L21, L192, L267).
  * Q16,K16: fp16 RoPE'd Q,K [B,H,N,D] (Qrope16/Krope16 of prepare_qk); V16: fp16 V [B,H,N,D]; fp32 accumulate.
  * workspace: required, >= rotattn_workspace_bytes(p,2). */

@@ -102,6 +102,16 @@ def rotattn_fwd_int4(p, Q4, Qs, K4, Ks, V4, Vs, O, workspace, ws_state, head_sel
           'rotattn_fwd_int4')
 
 
+def rotattn_fwd_int4_static(p, Q4, Qs, K4, Ks, V4, Vs, O, head_sel=None, stream=None):
+    """rotattn_fwd_int4 without a workspace argument, for callers that may not allocate device memory (a serving
+    process whose arena owns all of HBM, an operator with an inputs/outputs-only signature): the scratch is an 8 MiB
+    array inside librotattn.so.  Shapes whose workspace exceeds it raise; calls that overlap on the GPU race on it."""
+    _need_cuda(Q4, Qs, K4, Ks, V4, Vs, O, head_sel)
+    check(lib.rotattn_fwd_int4_static(C.byref(p), _ptr(Q4), _ptr(Qs), _ptr(K4), _ptr(Ks), _ptr(V4), _ptr(Vs), _ptr(O),
+                                      _ptr(head_sel), 0 if head_sel is None else head_sel.numel(), _stream(stream)),
+          'rotattn_fwd_int4_static')
+
+
 def rotattn_smooth_stats(p, coef_dev, rot_dev, Q, K, V, workspace, stream=None):
     _need_cuda(coef_dev, rot_dev, Q, K, V, workspace)
     check(lib.rotattn_smooth_stats(C.byref(p), _ptr(coef_dev), _ptr(rot_dev), _ptr(Q), _ptr(K), _ptr(V), _ptr(workspace),

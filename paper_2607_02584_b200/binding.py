@@ -14,6 +14,7 @@ P_ASYM15, P_SYM7 = 0, 1
 NORM_ROWBLOCK, NORM_RUNNING = 0, 1
 WS_HAS_QK, WS_HAS_V = 1, 2
 VSCALE_CHANNEL, VSCALE_GROUP = 0, 1
+STATIC_WS_BYTES = 8 << 20          # ROTATTN_STATIC_WS_BYTES of include/rotattn.h
 
 
 class RotattnParams(C.Structure):
@@ -48,6 +49,7 @@ EXPORTS = {
     'rotattn_prepare_qk': (C.c_int, [_P, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
     'rotattn_quant_v': (C.c_int, [_P, _vp, _vp, _vp, _vp, _sz, _vp]),
     'rotattn_fwd_int4': (C.c_int, [_P, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _i32, _vp, _sz, _i32, _vp]),
+    'rotattn_fwd_int4_static': (C.c_int, [_P, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _i32, _vp]),
     'rotattn_smooth_stats': (C.c_int, [_P, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
     'rotattn_smooth_read': (C.c_int, [_P, _vp, _sz, _vp, _vp, _vp]),
     'rotattn_fwd_int4_debug': (C.c_int, [_P, _vp, _vp, _vp, _vp, _vp, _vp, _i32, _i32, _vp, _vp, _vp, _vp, _vp, _sz, _i32, _vp]),
