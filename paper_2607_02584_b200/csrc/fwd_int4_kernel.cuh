@@ -256,7 +256,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     const int row = q0 + r;
     const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
     // Per-token: f = Qs_i * 2^18 log2e/sqrt(D); f >= 1e-30 keeps (-inf) * f well defined for masked keys; an all-zero
-    // query row still gives s == 0 everywhere.  QKG = 128: f = Qs_tile * Ks_block * 2^18 log2e/sqrt(D).
+    // query row still gives s == 0 everywhere.  QKG = 128: f = max(Qs_tile * Ks_block * 2^18 log2e/sqrt(D), 1e-30), same reason.
     float fq;
     if (QKG == 1) fq = (row < a.N) ? fmaxf(a.Qs[(size_t)bh * a.N + row] * a.scale_log2, 1e-30f) : 1e-30f;
     else fq = a.Qs[(size_t)bh * nblk + qtile] * a.scale_log2;
@@ -270,7 +270,7 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       const int ring = j % KS_RING, slot = j % P_SLOTS, abslot = j % AB_RING;
       const int nvalid = a.N - j * kTile;                  // < 128 only on the ragged last block
       float qs = fq;
-      if (QKG != 1) qs *= ksg[j];
+      if (QKG != 1) qs = fmaxf(qs * ksg[j], 1e-30f);       // a zero block scale (all-zero Q tile / K block) must not meet the -inf of masked keys
       const float2 qs2 = make_float2(qs, qs);
       if (QKG == 1) mbar_wait(&ks_full[ring], (j / KS_RING) & 1);
       mbar_wait(&s_done[j % K_STAGES], (j / K_STAGES) & 1);
@@ -493,8 +493,10 @@ int launch_one(const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& 
                cudaStream_t cs) {
   constexpr int smem = SmemInt4<D>::TOTAL;
   auto kern = fwd_int4_kernel<D, P_MODE, QKG, VSC, SM, PN, DEBUG>;
-  static int checked = 0;       // once per variant: ptxas must have allocated exactly the register pool setmaxnreg assumes
-  if (!checked) {
+  static PerDeviceOnce once;    // per variant and device: ptxas must have allocated exactly the register pool setmaxnreg assumes,
+  int dev = 0;                  // and the dynamic shared-memory opt-in is a per-device attribute
+  ROTATTN_CUDA_TRY(cudaGetDevice(&dev));
+  if (!once.done(dev)) {
     cudaFuncAttributes fa;
     ROTATTN_CUDA_TRY(cudaFuncGetAttributes(&fa, kern));
     if (fa.numRegs != 128) {
@@ -502,7 +504,7 @@ int launch_one(const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& 
       return ROTATTN_ERR_UNSUPPORTED;
     }
     ROTATTN_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    checked = 1;
+    once.mark(dev);
   }
   kern<<<grid, kFwdThreads, smem, cs>>>(tq, tk, tv, a);
   ROTATTN_CUDA_TRY(cudaGetLastError());

@@ -85,12 +85,33 @@ def test_granularity_variants_tiny_and_ragged(qk_group, v_scale, p_mode):
                 ph.check_tile(res, po, 0, h, qt, inputs=(pq['q_codes'], pq['q_scale'], pq['k_codes'], pq['k_scale'], vc, vs))
 
 
+@pytest.mark.parametrize('v_scale', [orc.VSCALE_CHANNEL, orc.VSCALE_GROUP])
+def test_zero_block_scales_at_ragged_n(v_scale):
+    """qk_group = 128 with an all-zero query tile and an all-zero valid part of the ragged last key block: both block
+    scales are exactly 0 (amax = 0 -> zeros), every score of those blocks is 0, and the keys >= N of the last
+    block are still masked - 0 * (-inf) must not reach the exponent."""
+    w = syn.small_variant(syn.HUNYUAN, (3, 9, 13), n_text=21, H=1)          # N = 372 = 2 * 128 + 116
+    q, k, v = syn.gen_all(w)
+    q, k = q.copy(), k.copy()
+    q[0, 0, 128:256] = 0
+    k[0, 0, 256:] = 0
+    res, po, tab = ph.run_path(w, q, k, v, rot_mode=orc.ROT_HALF, qk_group=128, v_scale=v_scale)
+    pq, vc, vs, _ = ph.check_prologue_head(po, tab, res, q[0, 0], k[0, 0], v[0, 0], 0, 0)
+    assert pq['q_scale'][1] == 0 and pq['k_scale'][2] == 0
+    assert bool(torch.isfinite(res['O'].float()).all())
+    for qt in range(3):
+        ph.check_tile(res, po, 0, 0, qt, inputs=(pq['q_codes'], pq['q_scale'], pq['k_codes'], pq['k_scale'], vc, vs))
+    ph.check_o(res['O'][0, 0].float().cpu().numpy(),
+               orc.o_quant(po, pq['q_codes'], pq['q_scale'], pq['k_codes'], pq['k_scale'], vc, vs))
+
+
 def test_fresh_workspace_unpack_path_and_head_sel():
     """fwd_int4 from the packed public buffers alone (ws_state = 0) and with a head subset."""
     api = ph.api()
     w = syn.small_variant(syn.WAN_1_3B, (2, 9, 13), H=3)
     q, k, v = syn.gen_all(w)
     res, po, tab = ph.run_path(w, q, k, v, rot_mode=orc.ROT_HALF, use_ws=False)
+    ph.check_prologue_head(po, tab, res, q[0, 1], k[0, 1], v[0, 1], 0, 1)     # the inputs taken from the GPU below are the oracle's
     qc, qs, kc, ks, vc, vs = ph.gpu_attention_inputs(res, 0, 1)
     ph.check_o(res['O'][0, 1].float().cpu().numpy(), orc.o_quant(po, qc, qs, kc, ks, vc, vs))
     b = res['buffers']
@@ -289,8 +310,9 @@ def test_d128_running_normaliser_ragged(p_mode):
     q, k, v = syn.gen_all(w)
     res, po, tab = ph.run_path(w, q, k, v, rot_mode=orc.ROT_HALF, p_mode=p_mode, p_norm=orc.NORM_RUNNING)
     for h in range(w.H):
+        pq, vc, vs, _ = ph.check_prologue_head(po, tab, res, q[0, h], k[0, h], v[0, h], 0, h)
         for qt in range(3):
-            ph.check_tile(res, po, 0, h, qt)
+            ph.check_tile(res, po, 0, h, qt, inputs=(pq['q_codes'], pq['q_scale'], pq['k_codes'], pq['k_scale'], vc, vs))
 
 
 def test_batch_of_two_and_d64_many_tiles():
