@@ -20,6 +20,14 @@ int rotattn_fwd_int4_debug(const rotattn_params* p,
                            int32_t bh, int32_t q_tile, int32_t* S_dump, uint8_t* P_dump, int32_t* PV_dump, void* O_tile,
                            void* workspace, size_t ws_bytes, int32_t ws_state, void* stream);
 
+/* rotattn_fwd_fp16 with the epilogue's quotient O/l stored as fp32 instead of being rounded to fp16 (same kernel, one
+ * compile-time switch in the last store).  It exists so that the kernel's ARITHMETIC can be held to north_star's strict
+ * "within 2e-3 max-abs of FP64 attention" (PAPER.md:L157 exact attention, L192 fallback precision): on the fp16 output half
+ * an ulp of |O| in [4, 16) is itself 2e-3 .. 3.9e-3, which is rounding of the result, not kernel error (reading 25).
+ * O32: out, fp32 [B,H,N,D], 16-byte aligned.  Other arguments as for rotattn_fwd_fp16. */
+int rotattn_fwd_fp16_debug_f32(const rotattn_params* p, const void* Q16, const void* K16, const void* V16, float* O32,
+                               const int32_t* head_sel, int32_t n_sel, void* workspace, size_t ws_bytes, void* stream);
+
 /* Dense 8-bit GEMM C[M,N] = A[M,K] * B[N,K]^T on the same tcgen05 path the attention kernel uses.
  * M multiple of 128, N multiple of 256, K multiple of 128.  A,B: device, row-major, 1 byte per element.
  *   mode 0: kind::i8, A and B signed int8, C int32.

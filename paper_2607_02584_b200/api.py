@@ -140,6 +140,16 @@ def rotattn_fwd_fp16(p, Q16, K16, V16, O, workspace, head_sel=None, stream=None)
                                workspace.numel() * workspace.element_size(), _stream(stream)), 'rotattn_fwd_fp16')
 
 
+def rotattn_fwd_fp16_debug_f32(p, Q16, K16, V16, O32, workspace, head_sel=None, stream=None):
+    """rotattn_debug.h: rotattn_fwd_fp16 with O/l stored as fp32 (test aid)."""
+    _need_cuda(Q16, K16, V16, O32, workspace, head_sel)
+    assert O32.dtype == torch.float32
+    check(lib.rotattn_fwd_fp16_debug_f32(C.byref(p), _ptr(Q16), _ptr(K16), _ptr(V16), _ptr(O32), _ptr(head_sel),
+                                         0 if head_sel is None else head_sel.numel(), _ptr(workspace),
+                                         workspace.numel() * workspace.element_size(), _stream(stream)),
+          'rotattn_fwd_fp16_debug_f32')
+
+
 def rotattn_probe_gemm8(M, N, K, A, B, Cout, mode=0, stream=None):
     _need_cuda(A, B, Cout)
     check(lib.rotattn_probe_gemm8(M, N, K, _ptr(A), _ptr(B), _ptr(Cout), mode, _stream(stream)), 'rotattn_probe_gemm8')

@@ -4,6 +4,7 @@
 #include <cuda_fp16.h>
 #include <stdint.h>
 #include <stddef.h>
+#include <atomic>
 #include "rotattn_debug.h"
 
 namespace rotattn {
@@ -64,6 +65,16 @@ int check_device_sm100();   // ROTATTN_OK or ROTATTN_ERR_UNSUPPORTED / ROTATTN_E
       return ROTATTN_ERR_CUDA;                                   \
     }                                                            \
   } while (0)
+
+// "Has the one-time set-up of this kernel run on device d?"  cudaFuncSetAttribute is per device (per context), so a flag
+// per process would leave the second GPU of a single-process multi-GPU host without its shared-memory opt-in.  One bit per
+// device ordinal; running the set-up twice from two racing host threads is harmless (it is idempotent), ordinals >= 64
+// simply repeat it on every launch.
+struct PerDeviceOnce {
+  std::atomic<uint64_t> bits{0};
+  bool done(int dev) const { return dev >= 0 && dev < 64 && ((bits.load(std::memory_order_acquire) >> dev) & 1u); }
+  void mark(int dev) { if (dev >= 0 && dev < 64) bits.fetch_or(uint64_t(1) << dev, std::memory_order_release); }
+};
 
 // internal launchers (prologue.cu)
 int launch_unpack_qk(const rotattn_params& p, const uint8_t* X4, int8_t* X8, cudaStream_t st);

@@ -25,6 +25,7 @@ constexpr int kFWarpAlloc = 12, kFWarpTma = 13, kFWarpMmaPV = 14, kFWarpMmaS = 1
 
 struct FwdFp16Args {
   __half* O;
+  float* O32;               // F32OUT flavour only (rotattn_debug.h): O/l before the rounding to fp16
   const int32_t* head_sel;
   int N, nblk;
   float scale_log2;
@@ -58,7 +59,7 @@ __device__ __forceinline__ uint32_t pack_half2(float lo, float hi) {
   return r;
 }
 
-template <int D>
+template <int D, bool F32OUT = false>
 __global__ void __launch_bounds__(kFp16Threads, 1)
 fwd_fp16_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                 const __grid_constant__ CUtensorMap tmV, const FwdFp16Args a) {
@@ -299,7 +300,16 @@ fwd_fp16_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         uint32_t v[32];
         tmem_ld32(tmem_base + lane_off + TM_O + x * 128 + cc * 32, v);
         tmem_wait_ld();
-        if (row < a.N) {
+        if (F32OUT) {                        // test flavour: the quotient itself, so that the kernel's arithmetic can be
+          if (row < a.N) {                   // held to the strict bound without the rounding of the fp16 output
+            float* dst = a.O32 + ((size_t)bh * a.N + row) * D + cc * 32;
+#pragma unroll
+            for (int d = 0; d < 32; d += 4)
+              *reinterpret_cast<float4*>(dst + d) =
+                  make_float4(__uint_as_float(v[d]) * inv_l, __uint_as_float(v[d + 1]) * inv_l,
+                              __uint_as_float(v[d + 2]) * inv_l, __uint_as_float(v[d + 3]) * inv_l);
+          }
+        } else if (row < a.N) {
           __half* dst = a.O + ((size_t)bh * a.N + row) * D + cc * 32;
 #pragma unroll
           for (int d = 0; d < 32; d += 8) {
@@ -343,28 +353,30 @@ __global__ void transpose_v_kernel(const __half* __restrict__ V, __half* __restr
 
 using namespace rotattn;
 
-template <int D>
+template <int D, bool F32OUT>
 static int launch_fp16(const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv, const FwdFp16Args& a, dim3 grid,
                        cudaStream_t cs) {
   constexpr int smem = SmemFp16<D>::TOTAL;
-  static int checked = 0;       // once: ptxas must have allocated exactly the register pool setmaxnreg redistributes
-  if (!checked) {
+  static PerDeviceOnce once;    // per device: ptxas must have allocated exactly the register pool setmaxnreg redistributes,
+  int dev = 0;                  // and the dynamic shared-memory opt-in is a per-device attribute
+  ROTATTN_CUDA_TRY(cudaGetDevice(&dev));
+  if (!once.done(dev)) {
     cudaFuncAttributes fa;
-    ROTATTN_CUDA_TRY(cudaFuncGetAttributes(&fa, fwd_fp16_kernel<D>));
+    ROTATTN_CUDA_TRY(cudaFuncGetAttributes(&fa, fwd_fp16_kernel<D, F32OUT>));
     if (fa.numRegs != 128) {
       set_error_text("fwd_fp16_kernel: unexpected register allocation (setmaxnreg pool assumes 128 registers per thread)");
       return ROTATTN_ERR_UNSUPPORTED;
     }
-    ROTATTN_CUDA_TRY(cudaFuncSetAttribute(fwd_fp16_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    checked = 1;
+    ROTATTN_CUDA_TRY(cudaFuncSetAttribute(fwd_fp16_kernel<D, F32OUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    once.mark(dev);
   }
-  fwd_fp16_kernel<D><<<grid, kFp16Threads, smem, cs>>>(tq, tk, tv, a);
+  fwd_fp16_kernel<D, F32OUT><<<grid, kFp16Threads, smem, cs>>>(tq, tk, tv, a);
   ROTATTN_CUDA_TRY(cudaGetLastError());
   return ROTATTN_OK;
 }
 
-extern "C" int rotattn_fwd_fp16(const rotattn_params* p, const void* Q16, const void* K16, const void* V16, void* O,
-                                const int32_t* head_sel, int32_t n_sel, void* workspace, size_t ws_bytes, void* stream) {
+static int fwd_fp16_common(const rotattn_params* p, const void* Q16, const void* K16, const void* V16, void* O, bool f32out,
+                           const int32_t* head_sel, int32_t n_sel, void* workspace, size_t ws_bytes, void* stream) {
   int st = rotattn_validate(p);
   if (st != ROTATTN_OK) return st;
   if (!Q16 || !K16 || !V16 || !O || !workspace) return ROTATTN_ERR_INVALID_ARG;
@@ -386,8 +398,21 @@ extern "C" int rotattn_fwd_fp16(const rotattn_params* p, const void* Q16, const 
   if ((st = make_tmap_3d(&tk, K16, 2, D, N, BH, D * 2, N * D * 2, 64, 128)) != ROTATTN_OK) return st;
   if ((st = make_tmap_3d(&tv, vt, 2, ws.npad, D, BH, (uint64_t)ws.npad * 2, D * ws.npad * 2, 64, (uint32_t)D)) != ROTATTN_OK) return st;
   FwdFp16Args a{};
-  a.O = (__half*)O; a.head_sel = head_sel; a.N = p->N; a.nblk = ceil_div(p->N, kTile);
+  a.O = f32out ? nullptr : (__half*)O; a.O32 = f32out ? (float*)O : nullptr;
+  a.head_sel = head_sel; a.N = p->N; a.nblk = ceil_div(p->N, kTile);
   a.scale_log2 = (float)(1.4426950408889634 / std::sqrt((double)p->D));
   dim3 grid(ceil_div(p->N, 2 * kTile), head_sel ? n_sel : BH);     // one CTA per pair of 128-row query tiles
-  return p->D == 128 ? launch_fp16<128>(tq, tk, tv, a, grid, cs) : launch_fp16<64>(tq, tk, tv, a, grid, cs);
+  if (f32out) return p->D == 128 ? launch_fp16<128, true>(tq, tk, tv, a, grid, cs) : launch_fp16<64, true>(tq, tk, tv, a, grid, cs);
+  return p->D == 128 ? launch_fp16<128, false>(tq, tk, tv, a, grid, cs) : launch_fp16<64, false>(tq, tk, tv, a, grid, cs);
+}
+
+extern "C" int rotattn_fwd_fp16(const rotattn_params* p, const void* Q16, const void* K16, const void* V16, void* O,
+                                const int32_t* head_sel, int32_t n_sel, void* workspace, size_t ws_bytes, void* stream) {
+  return fwd_fp16_common(p, Q16, K16, V16, O, false, head_sel, n_sel, workspace, ws_bytes, stream);
+}
+
+// rotattn_debug.h: the same kernel with O/l stored as fp32 (test aid, never on the timed path)
+extern "C" int rotattn_fwd_fp16_debug_f32(const rotattn_params* p, const void* Q16, const void* K16, const void* V16, float* O32,
+                                          const int32_t* head_sel, int32_t n_sel, void* workspace, size_t ws_bytes, void* stream) {
+  return fwd_fp16_common(p, Q16, K16, V16, O32, true, head_sel, n_sel, workspace, ws_bytes, stream);
 }
