@@ -24,6 +24,14 @@
 extern "C" {
 #endif
 
+/* Version of this binary interface.  It changes whenever a struct below gains, loses or moves a field or an enum value is
+ * renumbered (version 2 appended v_scale / smooth to rotattn_params, inserted n_heads into rotattn_policy and renumbered
+ * the `which` of rotattn_workspace_bytes; version 3 adds rotattn_fwd_int4_static and this query).  The structs carry no
+ * size field, so a caller built against another version would be read wrongly without any error: compare
+ * rotattn_abi_version() with the ROTATTN_ABI_VERSION you compiled against once, before the first other call. */
+#define ROTATTN_ABI_VERSION 3
+int rotattn_abi_version(void);
+
 typedef enum rotattn_status {
   ROTATTN_OK = 0,
   ROTATTN_ERR_INVALID_ARG = -1,         /* NULL pointer, sum(pairs) != D/2, t*h*w > N, n_sel out of range */

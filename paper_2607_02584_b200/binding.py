@@ -14,6 +14,7 @@ P_ASYM15, P_SYM7 = 0, 1
 NORM_ROWBLOCK, NORM_RUNNING = 0, 1
 WS_HAS_QK, WS_HAS_V = 1, 2
 VSCALE_CHANNEL, VSCALE_GROUP = 0, 1
+ABI_VERSION = 3                     # ROTATTN_ABI_VERSION this binding's struct layouts were written for
 STATIC_WS_BYTES = 8 << 20          # ROTATTN_STATIC_WS_BYTES of include/rotattn.h
 
 
@@ -38,6 +39,7 @@ lib = C.CDLL(LIB_PATH)
 _P = C.POINTER(RotattnParams)
 _vp, _sz, _i32 = C.c_void_p, C.c_size_t, C.c_int32
 EXPORTS = {
+    'rotattn_abi_version': (C.c_int, []),
     'rotattn_validate': (C.c_int, [_P]),
     'rotattn_table_floats': (_sz, [_P]),
     'rotattn_build_tables': (C.c_int, [_P, _vp, _vp]),
@@ -54,12 +56,18 @@ EXPORTS = {
     'rotattn_smooth_read': (C.c_int, [_P, _vp, _sz, _vp, _vp, _vp]),
     'rotattn_fwd_int4_debug': (C.c_int, [_P, _vp, _vp, _vp, _vp, _vp, _vp, _i32, _i32, _vp, _vp, _vp, _vp, _vp, _sz, _i32, _vp]),
     'rotattn_fwd_fp16': (C.c_int, [_P, _vp, _vp, _vp, _vp, _vp, _i32, _vp, _sz, _vp]),
+    'rotattn_fwd_fp16_debug_f32': (C.c_int, [_P, _vp, _vp, _vp, _vp, _vp, _i32, _vp, _sz, _vp]),
     'rotattn_probe_gemm8': (C.c_int, [_i32, _i32, _i32, _vp, _vp, _vp, _i32, _vp]),
 }
 for _name, (_res, _args) in EXPORTS.items():
     _fn = getattr(lib, _name)          # AttributeError here = the library does not export a declared symbol
     _fn.restype = _res
     _fn.argtypes = _args
+
+
+if lib.rotattn_abi_version() != ABI_VERSION:
+    raise ImportError(f'{LIB_PATH} speaks ABI version {lib.rotattn_abi_version()}, this binding was written for {ABI_VERSION}: '
+                      'rebuild with `python __graft_entry__.py`')
 
 
 class RotattnError(RuntimeError):

@@ -31,6 +31,8 @@ using namespace rotattn;
 
 extern "C" {
 
+int rotattn_abi_version(void) { return ROTATTN_ABI_VERSION; }
+
 int rotattn_validate(const rotattn_params* p) {
   if (!p) return ROTATTN_ERR_INVALID_ARG;
   if (p->B < 1 || p->H < 1 || p->N < 1) return ROTATTN_ERR_INVALID_ARG;

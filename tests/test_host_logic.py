@@ -25,6 +25,18 @@ def test_header_symbols_exported():
         assert hasattr(b.lib, n)
 
 
+def test_abi_version_matches_header_and_binding():
+    """The structs carry no size field: the version query is what tells a stale caller apart (include/rotattn.h)."""
+    hdr = open(os.path.join(ROOT, 'include', 'rotattn.h')).read()
+    ver = int(re.search(r'#define\s+ROTATTN_ABI_VERSION\s+(\d+)', hdr).group(1))
+    assert b.lib.rotattn_abi_version() == ver == b.ABI_VERSION
+    static = re.search(r'#define\s+ROTATTN_STATIC_WS_BYTES\s+\((\d+)u\s*<<\s*(\d+)\)', hdr)
+    assert int(static.group(1)) << int(static.group(2)) == b.STATIC_WS_BYTES
+    import ctypes as C
+    assert C.sizeof(b.RotattnParams) == 19 * 4          # 18 int32 + rope_base, no padding
+    assert C.sizeof(b.RotattnPolicy) == 7 * 4 + 4 + 8   # 7 int32, padding, one pointer
+
+
 def _p(w, **kw):
     return b.make_params(w.B, w.H, w.N, w.D, w.grid, w.pairs, **kw)
 

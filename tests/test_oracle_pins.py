@@ -357,6 +357,46 @@ def test_quantiser_properties():
     assert list(ct[0]) == [7, 0, 2, 2, 0, -2, 6, 3] and st[0] == 1.0
 
 
+def test_grouped_qk_quantiser_every_group():
+    """quant_qk(qk_group = 128) (north_star "per-block scales"; reading 28), checked group by group
+    on N = 300 = 128 + 128 + 44 (ragged last group) plus an all-zero middle group: scale = amax(group)/7 from an
+    independent slice, codes in [-7, 7], |y - code * scale| <= scale / 2, a +-7 in every non-zero group (at the position of
+    the group's amax), idempotence, and equality with the per-token routine on a hand-built equivalent problem.  A wrong
+    slice, a scale taken from another group or a ragged tail quantised with the wrong extent fails at least one."""
+    rng = np.random.default_rng(77)
+    N, D, G = 300, 64, 128
+    y = (rng.standard_normal((N, D)) * np.exp(rng.standard_normal((N, 1)))).astype(np.float32)
+    y[:G] *= 5.0                      # groups of clearly different magnitude: a scale borrowed from a neighbour breaks the error bound
+    y[2 * G:] *= 0.05
+    codes, scales = orc.quant_qk(y, G)
+    assert codes.shape == (N, D) and codes.dtype == np.int8 and scales.shape == (3,) and scales.dtype == np.float32
+    bounds = [(0, 128), (128, 256), (256, 300)]
+    for g, (lo, hi) in enumerate(bounds):
+        blk = y[lo:hi]
+        amax = np.abs(blk).max()
+        assert scales[g] == np.float32(amax / np.float32(7.0))                    # one fp32 division, of THIS group's amax
+        c = codes[lo:hi].astype(np.float32)
+        assert c.min() >= -7 and c.max() <= 7
+        assert np.all(np.abs(blk - c * scales[g]) <= scales[g] / 2 * (1 + 1e-6))
+        i, j = np.unravel_index(np.argmax(np.abs(blk)), blk.shape)
+        assert abs(int(codes[lo + i, j])) == 7 and np.sign(codes[lo + i, j]) == np.sign(blk[i, j])
+        # the same group as a per-token problem: a [1, n*D] row has the group's amax as its row amax
+        c1, s1 = orc.quant_qk(blk.reshape(1, -1))
+        assert np.array_equal(c1.reshape(blk.shape), codes[lo:hi]) and s1[0] == scales[g]
+    deq = np.concatenate([codes[lo:hi].astype(np.float32) * scales[g] for g, (lo, hi) in enumerate(bounds)])
+    c2, s2 = orc.quant_qk(deq, G)
+    assert np.array_equal(c2, codes) and np.allclose(s2, scales, rtol=1e-6)
+    # an all-zero group gives zero codes and a zero scale without touching its neighbours
+    yz = y.copy()
+    yz[G:2 * G] = 0.0
+    cz, sz = orc.quant_qk(yz, G)
+    assert sz[1] == 0 and not cz[G:2 * G].any()
+    assert np.array_equal(cz[:G], codes[:G]) and np.array_equal(cz[2 * G:], codes[2 * G:]) and sz[0] == scales[0] and sz[2] == scales[2]
+    # N an exact multiple of the group: no phantom group
+    c4, s4 = orc.quant_qk(y[:256], G)
+    assert s4.shape == (2,) and np.array_equal(c4, codes[:256]) and np.array_equal(s4, scales[:2])
+
+
 def test_v_group_quantiser():
     rng = np.random.default_rng(8)
     v = rng.standard_normal((300, 16)).astype(np.float16)
