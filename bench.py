@@ -9,7 +9,9 @@ The FP16 fallback kernel is timed beside it (speed-up denominator) but is not pa
 N > 1 (torchrun): every rank runs the full workload on its own GPU (independent (b,h) units, no collective);
 value = total ops of all ranks / max-over-ranks time ("weak").  `--head-shard` instead splits the heads of ONE workload
 over the ranks with paper_2607_02584_b200.dist.shard_heads ("strong").
-`--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload.
+`--gpus N` with N > 1 and no launcher (no WORLD_SIZE in the environment) starts the N ranks itself under torch.distributed.run.
+`--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload, `--steps` times after `--warmup`
+untimed samples; the sample (query rows per step) is sized from the first warm-up so that the whole run fits REFERENCE_BUDGET_S.
 """
 from __future__ import annotations
 
@@ -29,6 +31,7 @@ sys.path.insert(0, ROOT)
 
 METRIC = 'INT4 attn fwd effective TOPS (4*B*H*N^2*D ops per call; N=32760,H=12,D=128); ms/call in ms_per_step'
 WORKLOAD = 'wan1.3b-480p'
+REFERENCE_BUDGET_S = 150.0      # --impl reference: wall-clock budget of all its warm-up and timed samples together
 DTYPE = 'INT4 codes carried as exact E4M3 bytes (code * 2^-9) on tcgen05 kind::f8f6f4, fp32 accumulators holding the integers; fp32 softmax'
 
 
@@ -356,26 +359,70 @@ def variants_report(api, torch, w, Q, K, V, ops, iters):
         if t_stats is not None:
             out[name]['smooth_stats_ms'] = t_stats
         del bb
+    # SURVEY 8f row f4 as measurements: the same bytes seen as B = 2 x H/2 heads, and as 2H heads of D = 64 (the headline
+    # tensors reinterpreted - same value distribution, outlier channels land elsewhere; timing only, parity is in tests/)
+    from dataclasses import replace as _replace
+    B, H, N, D = w.B, w.H, w.N, w.D
+    shapes = [('shape_B2 (B=2, H=%d)' % (H // 2), _replace(w, B=2, H=H // 2), (2, H // 2, N, D)),
+              ('shape_D64 (H=%d, D=64, pairs 12/10/10)' % (2 * H), _replace(w, H=2 * H, D=64, pairs=(12, 10, 10)), (1, 2 * H, N, 64))]
+    for name, w2, shp in shapes:
+        p = api.params_for(w2, rot_mode=api.ROT_HALF)
+        cf = torch.from_numpy(api.rotattn_build_tables(p)).cuda()
+        bb = api.Buffers(p, want_fp16=True)
+        q2, k2, v2 = Q.view(shp), K.view(shp), V.view(shp)
+        t_prep = _time_ms(torch, lambda: api.rotattn_prepare_qk(p, cf, None, q2, k2, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.Q16, bb.K16, bb.ws), iters)
+        t_qv = _time_ms(torch, lambda: api.rotattn_quant_v(p, v2, bb.V4, bb.Vs, bb.ws), iters)
+        t = _time_ms(torch, lambda: api.rotattn_fwd_int4(p, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.V4, bb.Vs, bb.O, bb.ws, api.WS_HAS_QK | api.WS_HAS_V), iters, warm=2)
+        t16 = _time_ms(torch, lambda: api.rotattn_fwd_fp16(p, bb.Q16, bb.K16, v2, bb.O16, bb.ws16), max(2, iters // 2), warm=2)
+        ops2 = 4.0 * shp[0] * shp[1] * N * N * shp[3]
+        out[name] = {'fwd_int4_ms': t, 'tops': ops2 / t / 1e9, 'frac_of_2x_bf16_measured': ops2 / t / 1e9 / (2.0 * pk['bf16']),
+                     'prepare_qk_ms': t_prep, 'quant_v_ms': t_qv, 'fwd_fp16_ms': t16, 'fp16_tflops': ops2 / t16 / 1e9,
+                     'finite': bool(torch.isfinite(bb.O.float()).all()) and bool(torch.isfinite(bb.O16.float()).all())}
+        del bb
     return out
 
 
+def config_dict(w, world=1, head_shard=False):
+    """`config` of the JSON line - the same dict for both arms (the reference arm times a bounded sample of it)."""
+    return {'workload': WORKLOAD, 'B': w.B, 'H': w.H, 'N': w.N, 'D': w.D, 'grid': list(w.grid), 'rot_mode': 'HALF', 'p_mode': 'ASYM15',
+            'p_norm': 'ROWBLOCK', 'qk_group': 1, 'v_scale': 'per (128-token group, channel)',
+            'l2': 'inputs larger than L2 (Q,K,V fp16 = 302 MB per step; no flush)',
+            'parallelism': (f'heads sharded over {world} ranks, prologue included (no collective)' if head_shard and world > 1
+                            else f'replicas x{world} (independent (b,h) units, no collective)')}
+
+
 def run_reference(args):
+    """The oracle as it stands on the host cores: W untimed + K timed samples, every one the full prologue of one head
+    (N tokens) + quantised attention for `rows` query rows against all keys.  `rows` comes from the first warm-up sample
+    (256 rows) so that all W + K samples fit REFERENCE_BUDGET_S; it is the same for every sample of the run."""
     rank = int(os.environ.get('RANK', '0'))
     if rank != 0:
         return
-    steps, warm = args.steps, args.warmup
-    for _ in range(min(warm, 1)):
-        cpu_oracle_sample(256)
+    from synth import video_qkv as syn
+    K, W = max(1, args.steps), max(1, args.warmup)
+    t_start = time.perf_counter()
+    dt0, _, r0 = cpu_oracle_sample(256)                      # warm-up 1: also the calibration
+    dt1, _, r1 = cpu_oracle_sample(512)                      # warm-up 2 (counts only if W >= 2): separates prologue from per-row cost
+    per_row = max((dt1 - dt0) / max(r1 - r0, 1), 1e-6)
+    fixed = max(dt0 - per_row * r0, 0.0)
+    left = REFERENCE_BUDGET_S - (time.perf_counter() - t_start)
+    n_more = K + max(W - 2, 0)
+    rows = int((left / n_more - fixed) / per_row) // 128 * 128
+    rows = max(128, min(2048, rows))
+    for _ in range(max(W - 2, 0)):
+        cpu_oracle_sample(rows)
     ts, ops, nrows = [], 0.0, 0
-    for _ in range(max(1, min(steps, 3))):
-        dt, ops, nrows = cpu_oracle_sample(2048)
+    for _ in range(K):
+        dt, ops, nrows = cpu_oracle_sample(rows)
         ts.append(dt)
     dt = float(np.mean(ts))
     val = ops / dt / 1e12
-    sample = f'{WORKLOAD}: 1 head, full prologue on N=32760 tokens + O-quant for {nrows} query rows x all keys'
-    out = {'impl': 'reference', 'metric': METRIC, 'value': val, 'unit': 'TOPS', 'n_gpus': args.gpus, 'steps': len(ts),
-           'warmup': min(warm, 1), 'ms_per_step': dt * 1e3, 'higher_is_better': True, 'scaling': 'weak', 'vs_baseline': None,
-           'dtype': 'f64', 'data': 'synthetic', 'config': {'workload': WORKLOAD, 'note': 'bounded sample per step: ' + sample},
+    w = syn.ALL[WORKLOAD]
+    sample = (f'{WORKLOAD}: every step = 1 head, full prologue on N={w.N} tokens + O-quant for {nrows} query rows x all keys '
+              f'({K} timed steps after {max(W, 2)} warm-up samples, {time.perf_counter() - t_start:.0f} s in all)')
+    out = {'impl': 'reference', 'metric': METRIC, 'value': val, 'unit': 'TOPS', 'n_gpus': args.gpus, 'steps': K,
+           'warmup': max(W, 2), 'ms_per_step': dt * 1e3, 'higher_is_better': True, 'scaling': 'weak', 'vs_baseline': None,
+           'dtype': 'f64', 'data': 'synthetic', 'config': config_dict(w, args.gpus),
            'cpu_baseline': {'value': val, 'unit': 'TOPS', 'cores': os.cpu_count(), 'kind': 'oracle', 'sample': sample, 'cpu_model': _cpu_model()},
            'e2e': {'value': val, 'unit': 'TOPS', 'h2d_bytes_per_step': 0, 'd2h_bytes_per_step': 0}, 'gpu_launches': 0}
     print(json.dumps(out))
@@ -399,17 +446,23 @@ def main():
         print(json.dumps({'value': cops / dt / 1e12, 'unit': 'TOPS', 'threads': 1, 'rows': nrows, 'seconds': dt}))
         return
 
-    import torch
-    import torch.distributed as dist
     import __graft_entry__ as entry
     entry.build()
-    from paper_2607_02584_b200 import api
     from paper_2607_02584_b200 import dist as rdist
+    if rdist.needs_relaunch(args.gpus):          # `python bench.py --gpus N` without a launcher: start the N ranks here
+        sys.exit(rdist.relaunch_under_torchrun(args.gpus, os.path.abspath(__file__), sys.argv[1:]))
+    import torch
+    import torch.distributed as dist
+    from paper_2607_02584_b200 import api
     from synth import video_qkv as syn
 
     world = int(os.environ.get('WORLD_SIZE', '1'))
     rank = int(os.environ.get('RANK', '0'))
     local = int(os.environ.get('LOCAL_RANK', '0'))
+    if world != args.gpus:
+        raise SystemExit(f'--gpus {args.gpus} but the launcher started {world} rank(s)')
+    if local >= torch.cuda.device_count():
+        raise SystemExit(f'rank {rank}: no cuda:{local} on this node ({torch.cuda.device_count()} device(s) visible)')
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group('nccl', device_id=torch.device('cuda', local))
@@ -419,20 +472,29 @@ def main():
     p = api.params_for(w, rot_mode=api.ROT_HALF)
     B, H, N, D = w.B, w.H, w.N, w.D
     ops_full = 4.0 * B * H * N * N * D
-    # --head-shard: this rank's contiguous head range (no data-path collective)
+    # --head-shard: this rank's contiguous (b,h) range is a problem of its own - prologue, V quantiser and attention all run
+    # on the rank's slice only (B' = 1, H' = units owned), so nothing is replicated and there is no data-path collective
     head_sel = None
-    my_units = B * H
+    shard = None
     if args.head_shard and world > 1:
         mine = rdist.shard_heads(B * H, world, rank)
-        head_sel = torch.from_numpy(mine).cuda()
-        my_units = len(mine)
-    ops = ops_full * my_units / (B * H)
+        if len(mine) == 0:
+            raise SystemExit(f'--head-shard: rank {rank} of {world} owns no head of {B * H}')
+        shard = (int(mine[0]), int(mine[-1]) + 1)
+        ops = ops_full * len(mine) / (w.B * w.H)
+        from dataclasses import replace as _replace
+        p = api.params_for(_replace(w, B=1, H=len(mine)), rot_mode=api.ROT_HALF)
+        B, H = 1, len(mine)
+    else:
+        ops = ops_full
 
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
     # synthetic inputs of the BASELINE.json recipe (every replica runs the same seeded tensors)
     q, k, v = syn.gen_all(w)
+    if shard is not None:
+        q, k, v = (np.ascontiguousarray(x.reshape(w.B * w.H, N, D)[shard[0]:shard[1]][None]) for x in (q, k, v))
     hq, hk, hv = (torch.from_numpy(x).pin_memory() for x in (q, k, v))
     Q, Kt, V = hq.cuda(), hk.cuda(), hv.cuda()
     coef = torch.from_numpy(api.rotattn_build_tables(p)).cuda()
@@ -576,11 +638,7 @@ def main():
         'metric': METRIC, 'value': value_tops, 'unit': 'TOPS', 'n_gpus': world, 'steps': K, 'warmup': W,
         'ms_per_step': ms_step, 'higher_is_better': True, 'scaling': 'strong' if args.head_shard and world > 1 else 'weak',
         'vs_baseline': None, 'dtype': DTYPE, 'data': 'synthetic',
-        'config': {'workload': WORKLOAD, 'B': B, 'H': H, 'N': N, 'D': D, 'grid': list(w.grid), 'rot_mode': 'HALF', 'p_mode': 'ASYM15',
-                   'p_norm': 'ROWBLOCK', 'qk_group': 1, 'v_scale': 'per (128-token group, channel)',
-                   'l2': 'inputs larger than L2 (Q,K,V fp16 = 302 MB per step; no flush)',
-                   'parallelism': (f'heads sharded over {world} ranks (no collective)' if args.head_shard and world > 1
-                                   else f'replicas x{world} (independent (b,h) units, no collective)')},
+        'config': config_dict(w, world, args.head_shard),
         'kernels_ms': {'prepare_qk': t_prep, 'quant_v': t_qv, 'fwd_int4': t_int4, 'fwd_fp16': t_fp16},
         'step_as_cuda_graph_ms': graph_ms,
         'int4_kernel_tops': achieved, 'fp16_kernel_tflops': ops / (t_fp16 * 1e-3) / 1e12,
@@ -592,8 +650,11 @@ def main():
                          'peak': pk['hbm']},
         'roofline': {'kernel': 'fwd_int4_kernel', 'bound': 'tensor', 'achieved': achieved, 'peak': int8_peak, 'unit': 'TOPS',
                      'frac': achieved / int8_peak, 'traffic': traffic, 'traffic_source': traffic_src,
-                     'peak_source': f"2 x bf16_tflops ({pk['bf16']}) of {pk['src']} (dense 8-bit : bf16 nominal ratio 2; of measured)",
-                     'measured_8bit_gemm_peaks_this_run': peaks8},
+                     'peak_source': (f"NOMINAL ratio, not a measured 8-bit peak: 2 x bf16_tflops ({pk['bf16']}, burst) of {pk['src']} "
+                                     "(dense 8-bit : bf16 = 4.5 : 2.25 PFLOP/s nominal)"),
+                     'measured_8bit_gemm_peaks_this_run': peaks8,
+                     'frac_of_measured_f8f6f4_gemm_probe': (achieved / peaks8['probe_kind_f8f6f4_tops']
+                                                            if peaks8 and isinstance(peaks8.get('probe_kind_f8f6f4_tops'), float) else None)},
         'e2e': {'value': e2e_tops, 'unit': 'TOPS', 'ms_per_step': e2e_ms, 'how': 'C-ABI calls on pinned-host inputs; H2D / compute / D2H streams over double-buffered device tensors, every step copies all inputs in (Q, K, V staged in one pinned buffer, one transfer) and O out',
                 'h2d_bytes_per_step': h2d, 'd2h_bytes_per_step': d2h},
         'gpu_launches': 3 * K,

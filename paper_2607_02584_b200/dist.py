@@ -3,6 +3,11 @@ shards over contiguous head ranges with NO data-path collective; torch.distribut
 (max over ranks) and to gather per-rank results.  Pure host logic: works on the gloo backend without a GPU."""
 from __future__ import annotations
 
+import os
+import socket
+import subprocess
+import sys
+
 import numpy as np
 
 
@@ -38,3 +43,30 @@ def aggregate_throughput(units_done_local: float, ms_local: float, device='cpu')
         dist.all_reduce(t, op=dist.ReduceOp.SUM)
         total = float(t.item())
     return total / (ms * 1e-3)
+
+
+# ---- starting the ranks ------------------------------------------------------------------------------------------------
+def needs_relaunch(n_gpus: int, env=None) -> bool:
+    """`--gpus N` with N > 1 in a process that no launcher started (no WORLD_SIZE in the environment): the caller has to
+    start the N ranks itself.  Under torchrun (WORLD_SIZE set) the answer is False and the process is one of the ranks."""
+    env = os.environ if env is None else env
+    return n_gpus > 1 and 'WORLD_SIZE' not in env
+
+
+def torchrun_argv(n_gpus: int, script: str, script_args, port: int | None = None) -> list:
+    """The launch line of the bench contract: one process per GPU on this node, rendezvous on 127.0.0.1."""
+    if port is None:
+        with socket.socket() as sk:
+            sk.bind(('127.0.0.1', 0))
+            port = sk.getsockname()[1]
+    return [sys.executable, '-m', 'torch.distributed.run', '--nnodes=1', '--nproc-per-node', str(n_gpus),
+            '--master-addr', '127.0.0.1', '--master-port', str(port), script] + list(script_args)
+
+
+def relaunch_under_torchrun(n_gpus: int, script: str, script_args, env=None) -> int:
+    """Run `script` as n_gpus ranks and return the launcher's exit code (rank 0 prints the result line; the ranks'
+    stdout / stderr pass through).  NCCL's communicator log stays on so that the number of ranks can be read from it."""
+    env = dict(os.environ if env is None else env)
+    env.setdefault('NCCL_DEBUG', 'INFO')
+    env.setdefault('NCCL_DEBUG_SUBSYS', 'INIT')
+    return subprocess.call(torchrun_argv(n_gpus, script, script_args), env=env)

@@ -57,3 +57,21 @@ def test_shard_heads_properties():
             assert max(len(p) for p in parts) - min(len(p) for p in parts) <= 1
     with pytest.raises(ValueError):
         rd.shard_heads(4, 2, 2)
+
+
+def test_gpus_flag_starts_the_ranks_itself():
+    """`--gpus 2` without a launcher (no WORLD_SIZE): the program starts two ranks and ONE line comes out, saying 2."""
+    import json
+    import subprocess
+    import sys
+    from paper_2607_02584_b200 import dist as rd
+    assert rd.needs_relaunch(2, env={}) and not rd.needs_relaunch(1, env={}) and not rd.needs_relaunch(2, env={'WORLD_SIZE': '2'})
+    argv = rd.torchrun_argv(4, 'bench.py', ['--gpus', '4'], port=1234)
+    assert argv[1:] == ['-m', 'torch.distributed.run', '--nnodes=1', '--nproc-per-node', '4', '--master-addr', '127.0.0.1',
+                        '--master-port', '1234', 'bench.py', '--gpus', '4']
+    env = {k: v for k, v in os.environ.items() if k not in ('WORLD_SIZE', 'RANK', 'LOCAL_RANK', 'MASTER_ADDR', 'MASTER_PORT')}
+    probe = os.path.join(os.path.dirname(os.path.abspath(__file__)), 'spawn_probe.py')
+    r = subprocess.run([sys.executable, probe, '--gpus', '2'], env=env, capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [json.loads(x) for x in r.stdout.splitlines() if x.startswith('{')]
+    assert lines == [{'n_ranks': 2, 'units': 12, 'slowest_ms': 2.0}], r.stdout

@@ -229,20 +229,20 @@ def test_full_size_wan13b_row_sample():
         ph.check_o(res['O'][0, h].float().cpu().numpy()[rows], orc.o_quant(po, *inputs, rows=rows))
 
 
-def _full_size_case(w, heads, n_tiles=3, **modes):
+def _full_size_case(w, heads, n_tiles=3, bi=0, **modes):
     """Full N, D and ALL heads of a BASELINE.json config in one launch (the grid and workspace sizes bench.py uses).  For
-    the sampled heads: Q/K/V codes, scales and operand bytes against the oracle from the fp16 inputs (bit-exact), S / P /
-    P~V dumps on the ragged last tile, O on a seeded row sample."""
+    the sampled heads (of batch entry bi): Q/K/V codes, scales and operand bytes against the oracle from the fp16 inputs
+    (bit-exact), S / P / P~V dumps on the ragged last tile, O on a seeded row sample."""
     q, k, v = syn.gen_all(w)
     res, po, tab = ph.run_path(w, q, k, v, **modes)
-    assert res['O'].shape[1] == w.H
+    assert res['O'].shape[:2] == (w.B, w.H)
     for h in heads:
-        pq, vc, vs, _ = ph.check_prologue_head(po, tab, res, q[0, h], k[0, h], v[0, h], 0, h)
+        pq, vc, vs, _ = ph.check_prologue_head(po, tab, res, q[bi, h], k[bi, h], v[bi, h], bi, h)
         inputs = (pq['q_codes'], pq['q_scale'], pq['k_codes'], pq['k_scale'], vc, vs)
         rows = syn.sample_rows(w, n_tiles=n_tiles, head=h)
         tiles = sorted(set((rows // 128).tolist()))
-        ph.check_tile(res, po, 0, h, tiles[-1], inputs=inputs)
-        ph.check_o(res['O'][0, h].float().cpu().numpy()[rows], orc.o_quant(po, *inputs, rows=rows))
+        ph.check_tile(res, po, bi, h, tiles[-1], inputs=inputs)
+        ph.check_o(res['O'][bi, h].float().cpu().numpy()[rows], orc.o_quant(po, *inputs, rows=rows))
     # no head was left unwritten / non-finite
     assert bool(torch.isfinite(res['O'].float()).all())
     del res
@@ -279,6 +279,14 @@ def test_sweep_points_all_heads(idx):
 def test_sweep_naive_mode_and_granularity_variants_at_16384():
     _full_size_case(syn.SWEEP[1], [2], n_tiles=2, **NAIVE)
     _full_size_case(syn.SWEEP[1], [5], n_tiles=2, rot_mode=orc.ROT_HALF, qk_group=128, v_scale=orc.VSCALE_GROUP)
+
+
+def test_full_size_d64_and_batch_of_two():
+    """SURVEY 8f row f4 at the bench's N = 32760: D = 64 with 24 heads (pairs 12/10/10) and B = 2 (unit = b * H + h, the second
+    batch entry checked) - the two shapes bench.py times in its `variants` block."""
+    from dataclasses import replace
+    _full_size_case(replace(syn.WAN_1_3B, H=24, D=64, pairs=(12, 10, 10), name='wan1.3b-d64'), [0, 23], n_tiles=2, rot_mode=orc.ROT_HALF)
+    _full_size_case(replace(syn.WAN_1_3B, B=2, H=6, name='wan1.3b-b2'), [5], n_tiles=2, bi=1, rot_mode=orc.ROT_HALF)
 
 
 def test_mixed_precision_step_head_split():
