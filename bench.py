@@ -233,7 +233,7 @@ def quality_report(api, syn, torch, workloads, heads=(0, 1), n_tiles=2):
                 api.rotattn_smooth_stats(p, cf, None, Q, K, V, bb.ws)
             api.rotattn_prepare_qk(p, cf, None, Q, K, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.Q16, bb.K16, bb.ws)
             api.rotattn_quant_v(p, V, bb.V4, bb.Vs, bb.ws)
-            api.rotattn_fwd_int4(p, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.V4, bb.Vs, bb.O, bb.ws, api.WS_HAS_QK | api.WS_HAS_V)
+            api.rotattn_fwd_int4(p, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.V4, bb.Vs, bb.O, bb.ws, api.ws_state_full(p))
             torch.cuda.synchronize()
             o = np.concatenate([bb.O[0, i].float().cpu().numpy()[rows_h[i]] for i in range(len(hs))])
             entry[name] = metrics(o)
@@ -352,7 +352,7 @@ def variants_report(api, torch, w, Q, K, V, ops, iters):
             t_stats = _time_ms(torch, lambda: api.rotattn_smooth_stats(p, cf, None, Q, K, V, bb.ws), iters)
         t_prep = _time_ms(torch, lambda: api.rotattn_prepare_qk(p, cf, None, Q, K, bb.Q4, bb.Qs, bb.K4, bb.Ks, None, None, bb.ws), iters)
         t_qv = _time_ms(torch, lambda: api.rotattn_quant_v(p, V, bb.V4, bb.Vs, bb.ws), iters)
-        t = _time_ms(torch, lambda: api.rotattn_fwd_int4(p, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.V4, bb.Vs, bb.O, bb.ws, api.WS_HAS_QK | api.WS_HAS_V), iters, warm=2)
+        t = _time_ms(torch, lambda: api.rotattn_fwd_int4(p, bb.Q4, bb.Qs, bb.K4, bb.Ks, bb.V4, bb.Vs, bb.O, bb.ws, api.ws_state_full(p)), iters, warm=2)
         tops = ops / t / 1e9
         out[name] = {'fwd_int4_ms': t, 'tops': tops, 'frac_of_2x_bf16_measured': tops / (2.0 * pk['bf16']), 'prepare_qk_ms': t_prep,
                      'quant_v_ms': t_qv}

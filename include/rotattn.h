@@ -26,7 +26,7 @@ extern "C" {
 
 /* Version of this binary interface.  It changes whenever a struct below gains, loses or moves a field or an enum value is
  * renumbered (version 2 appended v_scale / smooth to rotattn_params, inserted n_heads into rotattn_policy and renumbered
- * the `which` of rotattn_workspace_bytes; version 3 adds rotattn_fwd_int4_static and this query).  The structs carry no
+ * the `which` of rotattn_workspace_bytes; version 3 adds rotattn_fwd_int4_static, ROTATTN_WS_HAS_STATS and this query).  The structs carry no
  * size field, so a caller built against another version would be read wrongly without any error: compare
  * rotattn_abi_version() with the ROTATTN_ABI_VERSION you compiled against once, before the first other call. */
 #define ROTATTN_ABI_VERSION 3
@@ -49,7 +49,11 @@ enum { ROTATTN_NORM_ROWBLOCK = 0, ROTATTN_NORM_RUNNING = 1 };
 enum { ROTATTN_VSCALE_CHANNEL = 0 /* one V scale per (128-token group, channel): DESIGN.md reading 11 */,
        ROTATTN_VSCALE_GROUP = 1   /* one V scale per 128-token group */ };
 /* ws_state bits for rotattn_fwd_int4 */
-enum { ROTATTN_WS_HAS_QK = 1, ROTATTN_WS_HAS_V = 2 };
+enum { ROTATTN_WS_HAS_QK = 1, ROTATTN_WS_HAS_V = 2,
+       ROTATTN_WS_HAS_STATS = 4 /* smooth = 1 only: the caller states that rotattn_smooth_stats ran on THIS workspace for THESE
+                                   Q, K, V before prepare_qk / quant_v.  The library cannot see it (it never reads device memory
+                                   on the host), and stale or missing means give a silently wrong O - so fwd_int4 refuses
+                                   smooth = 1 unless the caller has said so. */ };
 
 /* Problem statement: Q,K,V in R^{N x D} per head; D = D_f + D_h + D_w (L58);
  * block-diagonal rotation R of D/2 O(2) blocks (Eq.3); per-token Q/K and per-group V scales
@@ -177,7 +181,8 @@ int rotattn_smooth_read(const rotattn_params* p, const void* workspace, size_t w
  * head_sel: device int32 [n_sel] of b*H+h indices to process, or NULL (all B*H heads, n_sel ignored).
  * workspace: required, >= rotattn_workspace_bytes(p,1).  ws_state: ROTATTN_WS_HAS_QK|ROTATTN_WS_HAS_V
  *   if this workspace was passed to prepare_qk / quant_v with the same params; missing copies are rebuilt
- *   from the packed buffers by an unpack kernel first (smooth = 1 needs both bits: its state exists only there). */
+ *   from the packed buffers by an unpack kernel first (smooth = 1 needs both bits and ROTATTN_WS_HAS_STATS: its state
+ *   exists only there; anything less returns ROTATTN_ERR_INVALID_ARG). */
 int rotattn_fwd_int4(const rotattn_params* p,
                      const uint8_t* Q4, const float* Qs, const uint8_t* K4, const float* Ks,
                      const uint8_t* V4, const float* Vs, void* O,

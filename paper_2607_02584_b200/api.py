@@ -9,7 +9,7 @@ import torch
 
 from . import binding as _b
 from .binding import (ROT_NONE, ROT_INTERLEAVED, ROT_HALF, ROT_FULL, P_ASYM15, P_SYM7, NORM_ROWBLOCK, NORM_RUNNING,
-                      WS_HAS_QK, WS_HAS_V, VSCALE_CHANNEL, VSCALE_GROUP, make_params, check)
+                      WS_HAS_QK, WS_HAS_V, WS_HAS_STATS, VSCALE_CHANNEL, VSCALE_GROUP, make_params, check)
 
 lib = _b.lib
 
@@ -75,6 +75,11 @@ def rotattn_policy_split_heads(pol: dict, step: int, block: int, B: int, H: int)
     check(lib.rotattn_policy_split_heads(C.byref(st), step, block, B, H, _ptr(a), C.cast(C.byref(na), C.c_void_p),
                                          _ptr(b), C.cast(C.byref(nb), C.c_void_p)), 'rotattn_policy_split_heads')
     return a[:na.value].copy(), b[:nb.value].copy()
+
+
+def ws_state_full(p) -> int:
+    """ws_state of a workspace that went through the whole prologue for p (smooth_stats too when p.smooth)."""
+    return WS_HAS_QK | WS_HAS_V | (WS_HAS_STATS if p.smooth else 0)
 
 
 # ---- device entry points -------------------------------------------------------------------------
@@ -199,7 +204,7 @@ def run_int4(w, q, k, v, rot_mode=ROT_HALF, p_mode=P_ASYM15, p_norm=NORM_ROWBLOC
         rotattn_smooth_stats(p, coef_dev, rot_dev, Q, K, V, b.ws)
     rotattn_prepare_qk(p, coef_dev, rot_dev, Q, K, b.Q4, b.Qs, b.K4, b.Ks, b.Q16, b.K16, ws)
     rotattn_quant_v(p, V, b.V4, b.Vs, ws)
-    rotattn_fwd_int4(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, b.O, b.ws, (WS_HAS_QK | WS_HAS_V) if use_ws else 0)
+    rotattn_fwd_int4(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, b.O, b.ws, ws_state_full(p) if use_ws else 0)
     out = dict(p=p, Q4=b.Q4, K4=b.K4, V4=b.V4, Qs=b.Qs, Ks=b.Ks, Vs=b.Vs, O=b.O, buffers=b, coef=tab, V=V)
     if want_fp16:
         rotattn_fwd_fp16(p, b.Q16, b.K16, V, b.O16, b.ws16)

@@ -12,7 +12,7 @@ LIB_PATH = os.path.join(_HERE, 'librotattn.so')
 ROT_NONE, ROT_INTERLEAVED, ROT_HALF, ROT_FULL = 0, 1, 2, 3
 P_ASYM15, P_SYM7 = 0, 1
 NORM_ROWBLOCK, NORM_RUNNING = 0, 1
-WS_HAS_QK, WS_HAS_V = 1, 2
+WS_HAS_QK, WS_HAS_V, WS_HAS_STATS = 1, 2, 4
 VSCALE_CHANNEL, VSCALE_GROUP = 0, 1
 ABI_VERSION = 3                     # ROTATTN_ABI_VERSION this binding's struct layouts were written for
 STATIC_WS_BYTES = 8 << 20          # ROTATTN_STATIC_WS_BYTES of include/rotattn.h

@@ -20,8 +20,13 @@ int fwd_int4_common(const rotattn_params* p, const uint8_t* Q4, const float* Qs,
   const int nblk = ceil_div(p->N, kTile);
   if (head_sel && (n_sel < 1 || n_sel > BH)) return ROTATTN_ERR_INVALID_ARG;
   if (debug && (bh < 0 || bh >= BH || q_tile < 0 || q_tile >= nblk || !S_dump || !P_dump)) return ROTATTN_ERR_INVALID_ARG;
-  if (p->smooth && (ws_state & (ROTATTN_WS_HAS_QK | ROTATTN_WS_HAS_V)) != (ROTATTN_WS_HAS_QK | ROTATTN_WS_HAS_V))
-    return ROTATTN_ERR_INVALID_ARG;     // the smoothing state (means, per-key correction) exists only in the prologue's workspace
+  constexpr int kSmoothBits = ROTATTN_WS_HAS_QK | ROTATTN_WS_HAS_V | ROTATTN_WS_HAS_STATS;
+  if (p->smooth && (ws_state & kSmoothBits) != kSmoothBits) {
+    // the smoothing state (means, per-key correction) exists only in the prologue's workspace, and only if smooth_stats ran on it
+    set_error_text("rotattn_fwd_int4: smooth = 1 needs ws_state = HAS_QK | HAS_V | HAS_STATS (rotattn_smooth_stats, prepare_qk and "
+                   "quant_v must have run on this workspace)");
+    return ROTATTN_ERR_INVALID_ARG;
+  }
   WsInt4 ws(*p);
   if (ws_bytes < ws.total) return ROTATTN_ERR_WORKSPACE_TOO_SMALL;
   if ((st = check_device_sm100()) != ROTATTN_OK) return st;

@@ -130,7 +130,7 @@ def debug_tile(res, po, bh, q_tile, with_pv=True):
     PV = torch.zeros((nblk, 128, po.D), dtype=torch.int32, device='cuda') if with_pv else None
     Ot = torch.zeros((128, po.D), dtype=torch.float16, device='cuda')
     b = res['buffers']
-    a.rotattn_fwd_int4_debug(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, bh, q_tile, S, P, Ot, b.ws, a.WS_HAS_QK | a.WS_HAS_V,
+    a.rotattn_fwd_int4_debug(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, bh, q_tile, S, P, Ot, b.ws, a.ws_state_full(p),
                              PV_dump=PV)
     torch.cuda.synchronize()
     return S.cpu().numpy(), P.cpu().numpy(), None if PV is None else PV.cpu().numpy(), Ot.float().cpu().numpy()

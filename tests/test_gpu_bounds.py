@@ -79,7 +79,7 @@ def test_no_kernel_writes_outside_its_buffers(grid, n_text, base, qk_group, v_sc
         api.rotattn_smooth_stats(p, coef, None, Q, K, V, b.ws)
     api.rotattn_prepare_qk(p, coef, None, Q, K, b.Q4, b.Qs, b.K4, b.Ks, b.Q16, b.K16, b.ws)
     api.rotattn_quant_v(p, V, b.V4, b.Vs, b.ws)
-    api.rotattn_fwd_int4(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, b.O, b.ws, api.WS_HAS_QK | api.WS_HAS_V)
+    api.rotattn_fwd_int4(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, b.O, b.ws, api.ws_state_full(p))
     torch.cuda.synchronize()
     assert ar.guards_intact(), 'a kernel of the INT4 path wrote outside its buffers'
     o_first = b.O.clone()
