@@ -76,6 +76,51 @@ struct SmemInt4 {
   static constexpr int TOTAL = OFF_TMEM + 16;
 };
 
+// exp2 of a pair on the FMA pipe instead of the exp2 unit (MUFU.EX2 issues one warp instruction per 8 clk; where the
+// exp2 unit is the limiter a share of the exponentials is cheaper as arithmetic).  Cody-Waite: x = n + f with n = rne(x)
+// taken from the low mantissa bits of x + 1.5 * 2^23, f in [-0.5, 0.5]; 2^f by a minimax polynomial in relative error
+// (degree 4: 2.7e-6, degree 3: 7.5e-5, evaluated in fp32); 2^n by adding n to the exponent field.  Valid for
+// -125 <= x < 128; smaller arguments (masked keys carry -inf) are clamped, 2^-125 is 0 for every later use.
+#ifndef ROTATTN_POLY_DEG
+#define ROTATTN_POLY_DEG 3
+#endif
+__device__ __forceinline__ float2 ex2_fma_pipe2(float2 x) {
+  x.x = fmaxf(x.x, -125.f);
+  x.y = fmaxf(x.y, -125.f);
+  const float2 magic = make_float2(12582912.f, 12582912.f);
+  const float2 t = fadd2(x, magic);
+  const float2 n = fadd2(t, make_float2(-12582912.f, -12582912.f));
+  const float2 fr = ffma2(n, make_float2(-1.f, -1.f), x);
+#if ROTATTN_POLY_DEG == 4
+  float2 p = ffma2(make_float2(9.570101276e-03f, 9.570101276e-03f), fr, make_float2(5.591785908e-02f, 5.591785908e-02f));
+  p = ffma2(p, fr, make_float2(2.402474433e-01f, 2.402474433e-01f));
+  p = ffma2(p, fr, make_float2(6.931217909e-01f, 6.931217909e-01f));
+  p = ffma2(p, fr, make_float2(9.999992847e-01f, 9.999992847e-01f));
+#else
+  float2 p = ffma2(make_float2(5.517166480e-02f, 5.517166480e-02f), fr, make_float2(2.426111251e-01f, 2.426111251e-01f));
+  p = ffma2(p, fr, make_float2(6.932609677e-01f, 6.932609677e-01f));
+  p = ffma2(p, fr, make_float2(9.999280572e-01f, 9.999280572e-01f));
+#endif
+  return make_float2(__uint_as_float(__float_as_uint(p.x) + (__float_as_uint(t.x) << 23)),
+                     __uint_as_float(__float_as_uint(p.y) + (__float_as_uint(t.y) << 23)));
+}
+// Pairs per 16 keys (of 8) that take the FMA-pipe route.  Measured on cfg 2 (B200, round 3, ms per call):
+//   qk_group = 128 + v_scale = GROUP (the only variant the exp2 unit limits):
+//     0: 4.276   1 (deg 3): 4.159   2 (deg 3): 4.145 <- shipped   3 (deg 3): 4.430   4 (deg 3): 4.698   1 (deg 4): 4.171   2 (deg 4): 4.347
+//   qk_group = 128, per-channel V scales: 0: 4.514   1 (deg 4): 4.782   2 (deg 4): 4.989     (the drain's V-scale arithmetic already loads the FMA pipe)
+//   per-token Q/K scales: 0: 4.986 / 4.741 (v_scale = GROUP)   1 (deg 4): 5.015 / 4.703
+// so only the first gets it.  Degree 3 moves a P code by +-1 where LEVELS * P^ lies within ~1e-3 of a rounding boundary; the
+// parity tests hold the per-tile mismatch rate of this variant to the same 0.1 % as every other.
+#ifndef ROTATTN_POLY_BLOCK
+#define ROTATTN_POLY_BLOCK 2
+#endif
+#ifndef ROTATTN_POLY_BLOCK_VCH
+#define ROTATTN_POLY_BLOCK_VCH 0
+#endif
+#ifndef ROTATTN_POLY_TOKEN
+#define ROTATTN_POLY_TOKEN 0
+#endif
+
 template <int D, int P_MODE, int QKG, int VSC, int SM, int PN, bool DEBUG>
 __global__ void __launch_bounds__(kFwdThreads, 1)
 fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
@@ -364,8 +409,10 @@ fwd_int4_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           const uint32_t* w = &u[q >> 1][(q & 1) * 16 + x * 4];
           const float2 e0 = ffma2(make_float2(__uint_as_float(w[0]), __uint_as_float(w[1])), es2, nref2);
           const float2 e1 = ffma2(make_float2(__uint_as_float(w[2]), __uint_as_float(w[3])), es2, nref2);
+          constexpr int POLY = (QKG != 1 && VSC != 0) ? ROTATTN_POLY_BLOCK : (QKG != 1 ? ROTATTN_POLY_BLOCK_VCH : ROTATTN_POLY_TOKEN);
+          const bool poly = (POLY >= 1 && x == 3) || (POLY >= 2 && x == 1) || (POLY >= 3 && x == 2) || (POLY >= 4 && x == 0);   // compile-time after unrolling
           const float2 p0 = make_float2(ex2_approx(e0.x), ex2_approx(e0.y));
-          const float2 p1 = make_float2(ex2_approx(e1.x), ex2_approx(e1.y));
+          const float2 p1 = poly ? ex2_fma_pipe2(e1) : make_float2(ex2_approx(e1.x), ex2_approx(e1.y));
           ls0 = fadd2(ls0, p0);
           ls1 = fadd2(ls1, p1);
           const float2 f0 = fadd2(p0, magic2), f1 = fadd2(p1, magic2);

@@ -105,6 +105,23 @@ def test_zero_block_scales_at_ragged_n(v_scale):
                orc.o_quant(po, pq['q_codes'], pq['q_scale'], pq['k_codes'], pq['k_scale'], vc, vs))
 
 
+def test_smooth_needs_the_stats_bit():
+    """smooth = 1: fwd_int4 refuses a workspace the caller does not vouch for (ROTATTN_WS_HAS_STATS, include/rotattn.h) instead
+    of reading means nobody wrote."""
+    api = ph.api()
+    w = syn.small_variant(syn.WAN_1_3B, (2, 7, 11), H=1)
+    q, k, v = syn.gen_all(w)
+    res, po, tab = ph.run_path(w, q, k, v, rot_mode=orc.ROT_HALF, smooth=1)
+    b, p = res['buffers'], res['p']
+    for state in (0, api.WS_HAS_QK | api.WS_HAS_V, api.WS_HAS_STATS, api.WS_HAS_QK | api.WS_HAS_STATS):
+        with pytest.raises(RuntimeError, match='HAS_STATS'):
+            api.rotattn_fwd_int4(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, b.O, b.ws, state)
+    O2 = torch.zeros_like(b.O)
+    api.rotattn_fwd_int4(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, O2, b.ws, api.ws_state_full(p))
+    torch.cuda.synchronize()
+    assert torch.equal(O2, b.O)
+
+
 def test_fresh_workspace_unpack_path_and_head_sel():
     """fwd_int4 from the packed public buffers alone (ws_state = 0) and with a head subset."""
     api = ph.api()
@@ -123,18 +140,22 @@ def test_fresh_workspace_unpack_path_and_head_sel():
     assert torch.all(O2[0, 1] == 7.0)
 
 
-def test_diffuse_inputs_codes_cover_range():
-    """No outliers (diffuse attention): the case where P-code rounding matters most."""
+@pytest.mark.parametrize('qk_group,v_scale', [(1, orc.VSCALE_CHANNEL), (128, orc.VSCALE_GROUP)])
+def test_diffuse_inputs_codes_cover_range(qk_group, v_scale):
+    """No outliers (diffuse attention): the case where P-code rounding matters most - every key of a block lands on a
+    non-zero code.  The (128, GROUP) variant evaluates a quarter of its exponentials by a degree-3 polynomial on the FMA pipe
+    (fwd_int4_kernel.cuh): same +-1 / 0.1 % bound against the unchanged oracle."""
     w = syn.small_variant(syn.WAN_1_3B, (4, 8, 12), H=1)
     rng = np.random.default_rng(3)
     shape = (1, 1, w.N, w.D)
     q = (rng.standard_normal(shape) * 0.8).astype(np.float16)
     k = (rng.standard_normal(shape) * 0.8).astype(np.float16)
     v = rng.standard_normal(shape).astype(np.float16)
-    res, po, tab = ph.run_path(w, q, k, v, rot_mode=orc.ROT_HALF)
+    res, po, tab = ph.run_path(w, q, k, v, rot_mode=orc.ROT_HALF, qk_group=qk_group, v_scale=v_scale)
     stats = []
-    ph.check_tile(res, po, 0, 0, 1, stats=stats)
-    print(f'diffuse tile: P-code mismatch rate {stats[0]:.2e} (bound {ph.P_FRAC:.0e})')
+    for qt in range(3):
+        ph.check_tile(res, po, 0, 0, qt, stats=stats)
+    print(f'diffuse tiles (qk_group {qk_group}, v_scale {v_scale}): P-code mismatch rates {[f"{x:.2e}" for x in stats]} (bound {ph.P_FRAC:.0e})')
     _, P, _, _ = ph.debug_tile(res, po, 0, 0)
     assert set(np.unique(P[:, :w.N])) == set(range(16))
 
