@@ -468,7 +468,10 @@ __global__ void __launch_bounds__(256, 2) prepare_qk_kernel(const PrepArgs a) {
 // VSC = 1: one scale per group (the maximum over the channels as well).  SM = 1: v - column mean is quantised.
 // ------------------------------------------------------------------------------------------------
 template <int D, int VSC, int SM>
-__global__ void __launch_bounds__(256, 4) quant_v_kernel(const __half* __restrict__ V, uint8_t* __restrict__ V4,
+#ifndef ROTATTN_QV_MINBLOCKS
+#define ROTATTN_QV_MINBLOCKS 4
+#endif
+__global__ void __launch_bounds__(256, ROTATTN_QV_MINBLOCKS) quant_v_kernel(const __half* __restrict__ V, uint8_t* __restrict__ V4,
                                                       float* __restrict__ Vs, int8_t* __restrict__ V8T,
                                                       const float* __restrict__ means, int N, int nG, int npad) {
   constexpr int CR = D / 8;           // 16-byte chunks per row
