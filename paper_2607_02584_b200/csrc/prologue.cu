@@ -468,6 +468,8 @@ __global__ void __launch_bounds__(256, 2) prepare_qk_kernel(const PrepArgs a) {
 // VSC = 1: one scale per group (the maximum over the channels as well).  SM = 1: v - column mean is quantised.
 // ------------------------------------------------------------------------------------------------
 template <int D, int VSC, int SM>
+// 4 CTAs per SM cap the kernel at 64 registers (24 bytes of spill); 3 CTAs (80 registers, no spill) measure the same on cfg 2
+// (0.0496 vs 0.0497 ms per-channel, 0.0371 vs 0.0351 ms per-group): the spill is not the limiter (round 3).
 #ifndef ROTATTN_QV_MINBLOCKS
 #define ROTATTN_QV_MINBLOCKS 4
 #endif
