@@ -97,7 +97,7 @@ int rotattn_build_tables(const rotattn_params* p, const float* rot_host, float* 
 /* Bytes of scratch the device entry points need.  which = 0 (prepare_qk / quant_v / smooth_stats) and which = 1
  * (fwd_int4) are one and the same INT4-path workspace: sign-magnitude operand bytes of the Q/K codes [B,H,N,128] and
  * of the V codes transposed [B,H,D,ceil128(N)] (one byte per code = the E4M3 bit pattern of code * 2^-9), the key
- * scales padded to whole blocks, and the smoothing state.  which = 2: FP16 path (transposed V copy). */
+ * scales padded to whole blocks, and the smoothing state.  which = 2: FP16 path - 0 since ABI version 3 (V is read in place). */
 size_t rotattn_workspace_bytes(const rotattn_params* p, int which);
 
 /* Mixed-precision fallback policy: FP16 on the first/last sampling steps and the
@@ -217,7 +217,8 @@ int rotattn_fwd_int4_static(const rotattn_params* p,
 
 /* Step a10: FP16 FlashAttention forward, the fallback precision and the speed baseline (L21, L192, L267).
  * Q16,K16: fp16 RoPE'd Q,K [B,H,N,D] (Qrope16/Krope16 of prepare_qk); V16: fp16 V [B,H,N,D]; fp32 accumulate.
- * workspace: required, >= rotattn_workspace_bytes(p,2). */
+ * Q16, K16, V16, O: 16-byte aligned.  workspace / ws_bytes: ignored (kept for the ABI; the kernel needs no scratch: V is fed to the
+ * tensor cores as it lies in memory, as an MN-major operand); may be NULL / 0. */
 int rotattn_fwd_fp16(const rotattn_params* p, const void* Q16, const void* K16, const void* V16, void* O,
                      const int32_t* head_sel, int32_t n_sel,
                      void* workspace, size_t ws_bytes, void* stream);

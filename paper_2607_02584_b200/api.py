@@ -138,20 +138,22 @@ def rotattn_fwd_int4_debug(p, Q4, Qs, K4, Ks, V4, Vs, bh, q_tile, S_dump, P_dump
           'rotattn_fwd_int4_debug')
 
 
-def rotattn_fwd_fp16(p, Q16, K16, V16, O, workspace, head_sel=None, stream=None):
+def rotattn_fwd_fp16(p, Q16, K16, V16, O, workspace=None, head_sel=None, stream=None):
+    """workspace is ignored by the library since ABI version 3 (V is read in place); the parameter stays for old callers."""
     _need_cuda(Q16, K16, V16, O, workspace, head_sel)
     check(lib.rotattn_fwd_fp16(C.byref(p), _ptr(Q16), _ptr(K16), _ptr(V16), _ptr(O), _ptr(head_sel),
                                0 if head_sel is None else head_sel.numel(), _ptr(workspace),
-                               workspace.numel() * workspace.element_size(), _stream(stream)), 'rotattn_fwd_fp16')
+                               0 if workspace is None else workspace.numel() * workspace.element_size(), _stream(stream)),
+          'rotattn_fwd_fp16')
 
 
-def rotattn_fwd_fp16_debug_f32(p, Q16, K16, V16, O32, workspace, head_sel=None, stream=None):
+def rotattn_fwd_fp16_debug_f32(p, Q16, K16, V16, O32, workspace=None, head_sel=None, stream=None):
     """rotattn_debug.h: rotattn_fwd_fp16 with O/l stored as fp32 (test aid)."""
     _need_cuda(Q16, K16, V16, O32, workspace, head_sel)
     assert O32.dtype == torch.float32
     check(lib.rotattn_fwd_fp16_debug_f32(C.byref(p), _ptr(Q16), _ptr(K16), _ptr(V16), _ptr(O32), _ptr(head_sel),
                                          0 if head_sel is None else head_sel.numel(), _ptr(workspace),
-                                         workspace.numel() * workspace.element_size(), _stream(stream)),
+                                         0 if workspace is None else workspace.numel() * workspace.element_size(), _stream(stream)),
           'rotattn_fwd_fp16_debug_f32')
 
 

@@ -40,18 +40,6 @@ struct WsInt4 {
   }
 };
 
-// FP16-path workspace: V transposed [BH, D, npad] fp16.
-struct WsFp16 {
-  size_t vt, total;
-  int npad;
-  __host__ explicit WsFp16(const rotattn_params& p) {
-    size_t bh = (size_t)p.B * p.H;
-    npad = ceil_div(p.N, kTile) * kTile;
-    vt = 0;
-    total = align_up(bh * (size_t)p.D * npad * 2, 1024);
-  }
-};
-
 // error plumbing
 void set_cuda_error(cudaError_t e, const char* where);
 void set_error_text(const char* text);

@@ -1,7 +1,8 @@
 // rotattn_fwd_fp16 (step a10): FP16 FlashAttention forward on tcgen05 kind::f16 — the fallback precision
 // and the speed baseline the INT4 kernel is compared with (L267 "custom FP16 attention").
 //
-// One CTA = TWO 128-row query tiles (X = 0, 1) of one (b,h) sharing every K / V^T tile; 16 warps, warp-specialised:
+// One CTA = TWO 128-row query tiles (X = 0, 1) of one (b,h) sharing every K / V tile (V is read as it lies in memory,
+// [keys, D], as an MN-major B operand - no transposed copy); 16 warps, warp-specialised:
 //   warps 0-3 / 4-7  softmax group of tile 0 / 1: one thread per query row, the whole 128-key row of S in registers
 //                    (single pass over tensor memory), fp16 P written back over S (TMEM A operand of P V)
 //   warps 8-11       correction group: lazy rescale of the fp32 O accumulators that live in TMEM across KV blocks,
@@ -135,8 +136,8 @@ fwd_fp16_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         if (elect_one()) {
           mbar_arrive_expect_tx(&v_full[s], L::V_BYTES);
 #pragma unroll
-          for (int pn = 0; pn < 2; ++pn)      // key panels of 64
-            tma_load_3d(sV + s * L::V_BYTES + pn * (D * 128), &tmV, &v_full[s], j * kTile + pn * 64, 0, bh);
+          for (int pn = 0; pn < L::PANELS; ++pn)   // V as it lies in memory, [keys, D]: channel panels of 64, 128 keys each (keys >= N arrive as zeros)
+            tma_load_3d(sV + s * L::V_BYTES + pn * 16384, &tmV, &v_full[s], pn * 64, j * kTile, bh);
         }
         __syncwarp();
       }
@@ -169,7 +170,7 @@ fwd_fp16_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       }
     } else if (warp == kFWarpMmaPV) {
       // ---------------------------------------------------------------- MMA issuer 2: O_X += P_X(j) V(j)
-      constexpr uint32_t idesc_pv = umma_idesc(1, 0, 0, 128, D);
+      constexpr uint32_t idesc_pv = umma_idesc(1, 0, 0, 128, D) | (1u << 16);     // f32 <- f16 (TMEM) x f16, B MN-major
       for (int j = 0; j < nblk; ++j) {
         const int st = j % F_STAGES;
         mbar_wait(&v_full[st], (j / F_STAGES) & 1);
@@ -182,9 +183,9 @@ fwd_fp16_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             const uint32_t v_addr = smem_u32(sV + st * L::V_BYTES);
 #pragma unroll
             for (int kk = 0; kk < 8; ++kk) {
-              const uint32_t off = (kk >> 2) * (D * 128) + (kk & 3) * 32;
-              mma_ts<MmaKind::F16>(tmem_base + TM_O + x * 128, tmem_base + TM_S + x * 128 + 8 * kk, umma_desc_k128(v_addr + off),
-                                   idesc_pv, (j | kk) != 0);
+              // B operand = the V tile [128 keys, D], MN-major (D contiguous): 16 keys per step = two 8-row atoms
+              mma_ts<MmaKind::F16>(tmem_base + TM_O + x * 128, tmem_base + TM_S + x * 128 + 8 * kk,
+                                   umma_desc_mn128(v_addr + kk * 2048, 16384, 1024), idesc_pv, (j | kk) != 0);
             }
             tc_commit(&pv_done[x]);
             if (x == 1) tc_commit(&v_empty[st]);
@@ -329,26 +330,6 @@ fwd_fp16_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   if (warp == kFWarpAlloc) tmem_dealloc(tmem_base, 512);
 }
 
-// V [BH, N, D] fp16 -> V^T [BH, D, npad] fp16 (zero padded): K-major B operand of the P V product.
-__global__ void transpose_v_kernel(const __half* __restrict__ V, __half* __restrict__ VT, int N, int D, int npad) {
-  __shared__ __half tile[64][64 + 2];
-  const long long bh = blockIdx.z;
-  const int n0 = blockIdx.x * 64, d0 = blockIdx.y * 64;
-  for (int i = threadIdx.x; i < 64 * 32; i += blockDim.x) {
-    const int rr = i / 32, c2 = i % 32;
-    __half2 v = __floats2half2_rn(0.f, 0.f);
-    if (n0 + rr < N) v = *reinterpret_cast<const __half2*>(V + (bh * N + n0 + rr) * (long long)D + d0 + 2 * c2);
-    tile[rr][2 * c2] = __low2half(v);
-    tile[rr][2 * c2 + 1] = __high2half(v);
-  }
-  __syncthreads();
-  for (int i = threadIdx.x; i < 64 * 32; i += blockDim.x) {
-    const int dd = i / 32, n2 = i % 32;
-    __half2 v = __halves2half2(tile[2 * n2][dd], tile[2 * n2 + 1][dd]);
-    *reinterpret_cast<__half2*>(VT + (bh * D + d0 + dd) * (long long)npad + n0 + 2 * n2) = v;
-  }
-}
-
 }  // namespace rotattn
 
 using namespace rotattn;
@@ -379,24 +360,18 @@ static int fwd_fp16_common(const rotattn_params* p, const void* Q16, const void*
                            const int32_t* head_sel, int32_t n_sel, void* workspace, size_t ws_bytes, void* stream) {
   int st = rotattn_validate(p);
   if (st != ROTATTN_OK) return st;
-  if (!Q16 || !K16 || !V16 || !O || !workspace) return ROTATTN_ERR_INVALID_ARG;
+  if (!Q16 || !K16 || !V16 || !O) return ROTATTN_ERR_INVALID_ARG;
+  if (((uintptr_t)Q16 & 15) || ((uintptr_t)K16 & 15) || ((uintptr_t)V16 & 15) || ((uintptr_t)O & 15)) return ROTATTN_ERR_INVALID_ARG;   // TMA / 16-byte stores
+  (void)workspace; (void)ws_bytes;      // no scratch any more (V is read in place); the arguments stay for the ABI
   const int BH = p->B * p->H;
   if (head_sel && (n_sel < 1 || n_sel > BH)) return ROTATTN_ERR_INVALID_ARG;
-  WsFp16 ws(*p);
-  if (ws_bytes < ws.total) return ROTATTN_ERR_WORKSPACE_TOO_SMALL;
   if ((st = check_device_sm100()) != ROTATTN_OK) return st;
   cudaStream_t cs = (cudaStream_t)stream;
-  __half* vt = (__half*)((uint8_t*)workspace + ws.vt);
-  {
-    dim3 g(ws.npad / 64, p->D / 64, BH);
-    transpose_v_kernel<<<g, 256, 0, cs>>>((const __half*)V16, vt, p->N, p->D, ws.npad);
-    ROTATTN_CUDA_TRY(cudaGetLastError());
-  }
   const uint64_t N = p->N, D = p->D;
   CUtensorMap tq, tk, tv;
   if ((st = make_tmap_3d(&tq, Q16, 2, D, N, BH, D * 2, N * D * 2, 64, 128)) != ROTATTN_OK) return st;
   if ((st = make_tmap_3d(&tk, K16, 2, D, N, BH, D * 2, N * D * 2, 64, 128)) != ROTATTN_OK) return st;
-  if ((st = make_tmap_3d(&tv, vt, 2, ws.npad, D, BH, (uint64_t)ws.npad * 2, D * ws.npad * 2, 64, (uint32_t)D)) != ROTATTN_OK) return st;
+  if ((st = make_tmap_3d(&tv, V16, 2, D, N, BH, D * 2, N * D * 2, 64, 128)) != ROTATTN_OK) return st;
   FwdFp16Args a{};
   a.O = f32out ? nullptr : (__half*)O; a.O32 = f32out ? (float*)O : nullptr;
   a.head_sel = head_sel; a.N = p->N; a.nblk = ceil_div(p->N, kTile);

@@ -117,7 +117,7 @@ int rotattn_build_tables(const rotattn_params* p, const float* rot_host, float* 
 size_t rotattn_workspace_bytes(const rotattn_params* p, int which) {
   if (rotattn_validate(p) != ROTATTN_OK) return 0;
   if (which == 0 || which == 1) return WsInt4(*p).total;      // prepare_qk / quant_v and fwd_int4 share one workspace
-  if (which == 2) return WsFp16(*p).total;
+  if (which == 2) return 0;                                     // fwd_fp16 reads V in place (MN-major B operand): no scratch
   return 0;
 }
 

@@ -212,6 +212,20 @@ __device__ __forceinline__ uint64_t umma_desc_k128(uint32_t smem_addr) {
   return d;
 }
 
+// MN-major operand tile (the MN dimension is the contiguous one): rows of 128 bytes = 64 fp16 along MN, one row per k,
+// SWIZZLE_128B, 8 k-rows per 1024-byte atom (what a TMA box {64 elements of MN, rows of K} writes).  LBO = byte distance
+// between two 64-element MN panels, SBO = byte distance between two groups of 8 k-rows.  A K step of 16 advances the start
+// address by two atoms.  The instruction descriptor must carry the matching major bit (bit 16 for B).
+__device__ __forceinline__ uint64_t umma_desc_mn128(uint32_t smem_addr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  uint64_t d = 0;
+  d |= (uint64_t)((smem_addr & 0x3FFFFu) >> 4);
+  d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFFu) << 16;
+  d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFFu) << 32;
+  d |= (uint64_t)1 << 46;
+  d |= (uint64_t)2 << 61;
+  return d;
+}
+
 // Instruction descriptor (32 bit): [4,6) D format (0 f16, 1 f32, 2 s32) | [7,10) A format | [10,13) B format |
 // bit 15 A major (0 = K) | bit 16 B major | [17,23) N>>3 | [24,29) M>>4.
 // A/B format: kind::i8: 0 = u8, 1 = s8.  kind::f16: 0 = f16, 1 = bf16.  kind::f8f6f4: 0 = e4m3.

@@ -122,8 +122,7 @@ def test_workspace_too_small_is_reported():
     small = b.ws[:b.ws.numel() - 1]
     for call in (lambda: api.rotattn_prepare_qk(p, coef, None, Q, K, b.Q4, b.Qs, b.K4, b.Ks, None, None, small),
                  lambda: api.rotattn_quant_v(p, V, b.V4, b.Vs, small),
-                 lambda: api.rotattn_fwd_int4(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, b.O, small, 0),
-                 lambda: api.rotattn_fwd_fp16(p, b.Q16, b.K16, V, b.O16, b.ws16[:b.ws16.numel() - 1])):
+                 lambda: api.rotattn_fwd_int4(p, b.Q4, b.Qs, b.K4, b.Ks, b.V4, b.Vs, b.O, small, 0)):
         with pytest.raises(RuntimeError, match=r'workspace too small \(-4\)'):
             call()
 
